@@ -1,0 +1,198 @@
+/* triroof.h — C ABI of the B200-native (sm_100a) roofline microbenchmark and the two serving-phase
+ * kernels it stands in for, after "Energy-Efficient Multimodal Inference Serving with Tri-serve"
+ * (arxiv 2606.29629; text in PAPER.md).
+ *
+ * What the paper defines (citations are PAPER.md line numbers):
+ *   - a frequency-locked roofline microbenchmark: "a synthetic roofline kernel" swept across
+ *     arithmetic intensity (A.I., FLOP per byte) while throughput, power and core clock are
+ *     recorded (P:37-42 contribution 2, Sec. II-C.1, Sec. IV-A.3, Fig. 3 caption P:72);
+ *   - the two serving phases it stands in for: prefill = "dense GEMM kernels" with high A.I.,
+ *     decode = "GEMV-like operators" with low A.I. (P:90 Observation 2);
+ *   - per-phase SM clock / power observation and actuation through NVML,
+ *     nvmlDeviceSetGpuLockedClocks.
+ * BASELINE.json (north_star, configs 1-5) fixes the concrete operations; DESIGN.md lists every
+ * reading taken where the paper is silent.
+ *
+ * Conventions for every entry point:
+ *   - extern "C", returns an int status (TRI_OK == 0); no exception crosses the ABI;
+ *     tri_last_error() gives the detail text of the calling thread's last failure.
+ *   - "device pointer" = CUDA device memory of the current device, owned by the caller; the
+ *     library allocates no device memory per call (one lazily created 64-byte scratch excepted,
+ *     see tri_sm_clock_mhz) and never frees or retains caller buffers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream). Compute calls
+ *     validate their arguments on the host BEFORE any CUDA call, enqueue their kernel(s) on
+ *     `stream` and return; asynchronous faults surface at the caller's next synchronisation.
+ *   - There is no CPU fallback: a device that is not compute capability 10.x yields TRI_ERR_ARCH.
+ *   - bf16 values are passed as raw uint16_t bit patterns.
+ */
+#ifndef TRIROOF_H_
+#define TRIROOF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    TRI_OK = 0,
+    TRI_ERR_INVALID_ARG = 1,       /* null pointer, non-positive size, ai not a multiple of 1/4, partial overlap */
+    TRI_ERR_UNSUPPORTED_SHAPE = 2, /* shape outside what the kernels cover (no silent fallback) */
+    TRI_ERR_ALIGNMENT = 3,         /* pointer or leading dimension not aligned as stated below */
+    TRI_ERR_CUDA = 4,              /* a CUDA runtime / driver call failed; see tri_last_error() */
+    TRI_ERR_ARCH = 5,              /* device is not compute capability 10.x */
+    TRI_ERR_NVML_UNAVAILABLE = 6,  /* libnvidia-ml.so.1 could not be loaded or initialised */
+    TRI_ERR_NO_PERMISSION = 7,     /* NVML refused a clock lock (a normal outcome in containers) */
+    TRI_ERR_BUFFER_TOO_SMALL = 8   /* sample / summary capacity exhausted; output truncated */
+};
+
+/* Physical layout of the weight operand W (logical shape W[k][n], value at (k, n) independent of layout). */
+enum {
+    TRI_W_NK = 0, /* W_phys[n * ldw + k], K contiguous, ldw >= k   (nn.Linear storage; the reported path) */
+    TRI_W_KN = 1  /* W_phys[k * ldw + n], N contiguous, ldw >= n   ("[3584 x 18944]" as BASELINE.json writes it) */
+};
+
+/* Static string for a status code (never NULL). */
+const char *tri_status_string(int status);
+/* Thread-local detail of the calling thread's most recent failure ("" if none). Valid until that
+ * thread's next failing call. */
+const char *tri_last_error(void);
+
+/* Selects `device` (cudaSetDevice), checks it is cc 10.x, caches SM count / L2 size.
+ * Idempotent; the compute calls call it lazily with the current device. */
+int tri_init(int device);
+/* Resets clocks this process locked through tri_lock_clocks, releases NVML and the scratch buffer. */
+void tri_shutdown(void);
+/* Cached device facts (0 before a successful tri_init). */
+int tri_sm_count(void);
+size_t tri_l2_bytes(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * a1. A.I.-parameterised FMA-chain streaming kernel — the roofline microbenchmark
+ *     ("synthetic roofline kernel"; BASELINE.json configs 1-2).
+ *
+ *     for i in [0, n):  y = in[i];  repeat k times: y = fmaf(a, y, b);  out[i] = y
+ *
+ * fp32, IEEE round-to-nearest-even, fused (one rounding per step), steps in this order; the result
+ * is bit-exact against the CPU definition.  Per element: 4 B read + 4 B written and 2k FLOP, so
+ * A.I. = 2k/8 = k/4 FLOP/B.
+ *
+ * roofline_run:   ai in FLOP/byte; k = 4*ai must be an integer in [1, 2^20] (|4ai - round(4ai)| <
+ *                 1e-9) else TRI_ERR_INVALID_ARG.  Uses a = 0.9990234375, b = 0.0009765625
+ *                 (BASELINE.json config 1).
+ * roofline_run_k: explicit k in [1, 2^20] and explicit a, b.
+ * n:   number of elements, any value >= 0 (n == 0 enqueues nothing and returns TRI_OK).
+ * in:  device pointer, n floats, 16-byte aligned.   out: device pointer, n floats, 16-byte aligned.
+ *      in == out is allowed (each element is read, then written, by the same thread); any other
+ *      overlap of [in, in+n) and [out, out+n) is TRI_ERR_INVALID_ARG.
+ * Asynchronous: one kernel on `stream`.
+ */
+int roofline_run(double ai, size_t n, const float *in, float *out, void *stream);
+int roofline_run_k(unsigned k, float a, float b, size_t n, const float *in, float *out, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a2. Decode-phase GEMV ("GEMV-like operators", memory-bound; BASELINE.json config 3).
+ *
+ *     Y[i][j] = bf16_rne( sum_k float(X[i][k]) * float(W[k][j]) ),  fp32 accumulation (any order)
+ *
+ * m: rows of X, 1 <= m <= 16 (the decode batch).  n: columns of W, >= 1.  k: inner size, >= 8,
+ * k % 8 == 0.  x: device, bf16 X[i * ldx + kk], ldx >= k, ldx % 8 == 0.
+ * w: device, bf16, layout w_layout (TRI_W_NK: ldw >= k; TRI_W_KN: ldw >= n), ldw % 8 == 0.
+ * y: device, bf16 Y[i * ldy + j], ldy >= n.  x, w 16-byte aligned; y 2-byte aligned (any ldy).
+ * Outputs must not alias inputs.  Asynchronous: one kernel per 8 rows of X on `stream`.
+ */
+int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw,
+                int w_layout, uint16_t *y, int64_t ldy, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a3. Prefill-phase GEMM ("dense GEMM kernels", compute-bound; BASELINE.json config 4).
+ *
+ *     C[i][j] = bf16_rne( sum_k float(A[i][k]) * float(W[k][j]) ),  fp32 accumulation in tensor
+ *     memory (tcgen05.mma kind::f16), operands staged by TMA.
+ *
+ * m, n >= 1; k >= 8, k % 8 == 0.  a: device bf16 A[i * lda + kk], lda >= k, lda % 8 == 0.
+ * w: as in decode_gemv.  c: device bf16 C[i * ldc + j], ldc >= n, ldc % 8 == 0.
+ * a, w, c 16-byte aligned.  Ragged m, n, k tiles are handled inside (TMA zero fill, clipped stores).
+ * Outputs must not alias inputs.  Asynchronous: one kernel on `stream`.
+ */
+int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
+                 int w_layout, uint16_t *c, int64_t ldc, void *stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a4. Phase trace (Fig. 1 bottom, Fig. 4a, P:124 NVML, P:126 event-anchored phase
+ *     boundaries; BASELINE.json config 5).  All buffers here are HOST memory owned by the caller.
+ */
+typedef struct {
+    double t_s;                 /* CLOCK_MONOTONIC seconds since phase_trace_start */
+    int32_t phase;              /* tag current when the sample was taken */
+    uint32_t sm_mhz, mem_mhz;   /* nvmlDeviceGetClockInfo(SM / MEM) */
+    uint32_t temp_c;            /* GPU temperature */
+    float power_w;              /* nvmlDeviceGetPowerUsage / 1000 */
+    uint64_t energy_mj;         /* nvmlDeviceGetTotalEnergyConsumption (0 if unsupported) */
+    uint64_t clk_event_reasons; /* nvmlDeviceGetCurrentClocksEventReasons bitmask */
+} tri_sample;
+
+typedef struct {
+    int32_t phase;              /* TRI_PHASE_* */
+    int32_t reserved;
+    double t_begin_s, t_end_s;  /* host clock, same origin as tri_sample.t_s */
+    double gpu_ms;              /* cudaEvent time between the phase's first and last kernel (0 for idle) */
+    uint64_t launches;          /* kernel launches completed in the phase */
+    double flop, bytes, tokens; /* algorithmic work done (tokens: m per call) */
+    double energy_j, mean_power_w, j_per_flop, j_per_byte, j_per_token;
+    float sm_mhz_mean, sm_mhz_first10, sm_mhz_last10; /* clock over the phase / its first, last 10 % */
+    float temp_c_max;
+    uint32_t n_samples;
+    uint32_t reserved2;
+} tri_phase_summary;
+
+enum { TRI_PHASE_IDLE = 0, TRI_PHASE_PREFILL = 1, TRI_PHASE_DECODE = 2, TRI_PHASE_ROOFLINE = 3 };
+
+/* Low-level sampler: a host thread polls NVML every period_us (>= 1000) into buf[0..cap), tagging
+ * each sample with the current phase.  *handle receives an opaque pointer.  When cap is reached
+ * sampling stops silently and phase_trace_stop returns TRI_ERR_BUFFER_TOO_SMALL (data kept). */
+int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t cap, void **handle);
+int phase_trace_mark(void *handle, int phase); /* atomic tag switch; any thread */
+int phase_trace_stop(void *handle, size_t *n_samples); /* joins the sampler thread, frees the handle */
+
+/* Caller-owned DEVICE buffers and shapes for the two phase kernels. */
+typedef struct {
+    int pm, pn, pk;             /* prefill GEMM shape (config 4: 4096, 18944, 3584) */
+    const uint16_t *pa;         /* A [pm][pk] bf16, lda = pk */
+    const uint16_t *pw;         /* W, layout w_layout, ld = pk (NK) or pn (KN) */
+    uint16_t *pc;               /* C [pm][pn] bf16, ldc = pn */
+    int dm, dn, dk;             /* decode GEMV shape (config 3: 8, 18944, 3584) */
+    const uint16_t *dx;         /* X [dm][dk] */
+    const uint16_t *const *dw_ring; /* HOST array of dw_count device pointers: rotating weight copies */
+    int dw_count;               /* >= 1; rotate so the stream stays HBM-resident, not L2-resident */
+    uint16_t *dy;               /* Y [dm][dn] */
+    int w_layout;
+    void *stream;
+} tri_trace_workload;
+
+/* Config-5 driver (blocking; runs on the calling host thread): repeats
+ * [prefill GEMM for prefill_s | decode GEMV for decode_s | idle for idle_s] until total_s has
+ * elapsed, sampling NVML every period_ms.  Kernels are launched back to back with a bounded queue
+ * depth; the idle phase launches nothing and blocks the host thread (stands in for the sem_wait
+ * dependency stall).  samples[0..cap) / summaries[0..scap) are filled; the counts
+ * are returned through n_samples / n_summaries. */
+int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, double decode_s,
+                double idle_s, unsigned period_ms, tri_sample *samples, size_t cap, size_t *n_samples,
+                tri_phase_summary *summaries, size_t scap, size_t *n_summaries);
+
+/* NVML actuation primitive of the paper.  TRI_ERR_NO_PERMISSION is a normal outcome. */
+int tri_lock_clocks(int device, unsigned sm_mhz, unsigned mem_mhz); /* mem_mhz == 0: leave memory clock */
+int tri_reset_clocks(int device);
+
+/* One NVML reading outside a trace (phase = -1). */
+int tri_nvml_sample(int device, tri_sample *out);
+
+/* SM clock seen from inside the GPU: a one-block kernel spins for about spin_us microseconds and
+ * returns delta(clock64) / delta(globaltimer ns) * 1000 in *mhz.  Blocking (synchronises stream). */
+int tri_sm_clock_mhz(unsigned spin_us, double *mhz, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRIROOF_H_ */

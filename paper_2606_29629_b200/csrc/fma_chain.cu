@@ -1,0 +1,155 @@
+// a1. A.I.-parameterised FMA-chain streaming kernel (the roofline microbenchmark; PAPER.md lines 92,
+// 205; BASELINE.json configs 1-2; ABI in include/triroof.h).
+//
+//   out[i] = chain_k(in[i]),  chain: y <- fmaf(a, y, b) repeated k times, fp32 RN, fused.
+//
+// Layout: a tile is THREADS * VEC float4 (coalesced: float4 j of thread t sits at tile + j*THREADS + t).
+// Every thread carries VEC*4 independent chains (VEC*2 packed FFMA2 chains), which hides the FFMA
+// latency at the compute end; at the memory end all VEC 128-bit loads are issued before the first
+// FMA.  The k loop is a runtime loop (k is arbitrary, not a power of two) unrolled by 8 with a
+// remainder loop.  __ffma2_rn is, per component, __fmaf_rn (crt/sm_100_rt.h), so packing two chains
+// in one instruction does not change a bit; no fast-math, no FTZ.
+#include "tri_internal.h"
+
+#include <cmath>
+#include <cstdlib>
+
+namespace tri {
+
+constexpr int FMA_THREADS = 256;
+
+__device__ __forceinline__ float4 ld_stream(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.cs.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream(float4 *p, const float4 &v)
+{
+    asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+template <int NPAIR>
+__device__ __forceinline__ void chain_steps(float2 (&y)[NPAIR], unsigned k, float a, float b)
+{
+    const float2 a2 = make_float2(a, a), b2 = make_float2(b, b);
+    unsigned s = k;
+#pragma unroll 1
+    for (; s >= 8; s -= 8) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+#pragma unroll
+            for (int j = 0; j < NPAIR; ++j) y[j] = __ffma2_rn(a2, y[j], b2);
+    }
+#pragma unroll 1
+    for (; s > 0; --s) {
+#pragma unroll
+        for (int j = 0; j < NPAIR; ++j) y[j] = __ffma2_rn(a2, y[j], b2);
+    }
+}
+
+// n4 = number of whole float4 groups; `tail` (< 4) scalars follow them and are done by block 0.
+template <int VEC>
+__global__ void __launch_bounds__(FMA_THREADS)
+fma_chain_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n4, unsigned tail, unsigned k, float a, float b)
+{
+    const float4 *in4 = reinterpret_cast<const float4 *>(in);
+    float4 *out4 = reinterpret_cast<float4 *>(out);
+    const size_t tile = (size_t)blockIdx.x * (FMA_THREADS * VEC);
+    const size_t base = tile + threadIdx.x;
+
+    if (tile + (size_t)FMA_THREADS * VEC <= n4) {           // full tile: no predicates
+        float2 y[VEC * 2];
+#pragma unroll
+        for (int j = 0; j < VEC; ++j) {
+            float4 v = ld_stream(in4 + base + (size_t)j * FMA_THREADS);
+            y[2 * j] = make_float2(v.x, v.y);
+            y[2 * j + 1] = make_float2(v.z, v.w);
+        }
+        chain_steps<VEC * 2>(y, k, a, b);
+#pragma unroll
+        for (int j = 0; j < VEC; ++j)
+            st_stream(out4 + base + (size_t)j * FMA_THREADS, make_float4(y[2 * j].x, y[2 * j].y, y[2 * j + 1].x, y[2 * j + 1].y));
+    } else {                                                 // ragged last tile
+#pragma unroll 1
+        for (int j = 0; j < VEC; ++j) {
+            size_t idx = base + (size_t)j * FMA_THREADS;
+            if (idx < n4) {
+                float4 v = in4[idx];
+                float2 y[2] = {make_float2(v.x, v.y), make_float2(v.z, v.w)};
+                chain_steps<2>(y, k, a, b);
+                out4[idx] = make_float4(y[0].x, y[0].y, y[1].x, y[1].y);
+            }
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x < tail) {            // scalar tail (n % 4 elements)
+        size_t i = n4 * 4 + threadIdx.x;
+        float y = in[i];
+#pragma unroll 1
+        for (unsigned s = 0; s < k; ++s) y = __fmaf_rn(a, y, b);
+        out[i] = y;
+    }
+}
+
+template <int VEC>
+static cudaError_t launch(const float *in, float *out, size_t n, unsigned k, float a, float b, cudaStream_t s)
+{
+    size_t n4 = n / 4;
+    unsigned tail = (unsigned)(n % 4);
+    size_t per = (size_t)FMA_THREADS * VEC;
+    size_t blocks = (n4 + per - 1) / per;
+    if (blocks == 0) blocks = 1;   // tail only
+    fma_chain_kernel<VEC><<<(unsigned)blocks, FMA_THREADS, 0, s>>>(in, out, n4, tail, k, a, b);
+    return cudaGetLastError();
+}
+
+static int run(unsigned k, float a, float b, size_t n, const float *in, float *out, void *stream)
+{
+    if (k < 1 || k > (1u << 20)) return fail(TRI_ERR_INVALID_ARG, "k = %u outside [1, 2^20]", k);
+    if (n == 0) return TRI_OK;
+    if (!in || !out) return fail(TRI_ERR_INVALID_ARG, "in/out is NULL");
+    if (!aligned(in, 16) || !aligned(out, 16)) return fail(TRI_ERR_ALIGNMENT, "in/out must be 16-byte aligned");
+    if (n > ((size_t)1 << 40)) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "n = %zu exceeds 2^40", n);
+    if (in != out) {
+        uintptr_t i0 = (uintptr_t)in, o0 = (uintptr_t)out, bytes = n * sizeof(float);
+        if (i0 < o0 + bytes && o0 < i0 + bytes) return fail(TRI_ERR_INVALID_ARG, "in and out overlap partially");
+    }
+    int st = ensure_init(nullptr);
+    if (st != TRI_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    static int variant = -1;                                 // debug override only: TRI_FMA_VEC in {1, 2, 4, 8}
+    if (variant < 0) {
+        const char *e = getenv("TRI_FMA_VEC");
+        variant = e ? atoi(e) : 0;
+    }
+    int vec = variant ? variant : 4;
+    cudaError_t e;
+    switch (vec) {
+        case 1: e = launch<1>(in, out, n, k, a, b, s); break;
+        case 2: e = launch<2>(in, out, n, k, a, b, s); break;
+        case 8: e = launch<8>(in, out, n, k, a, b, s); break;
+        default: e = launch<4>(in, out, n, k, a, b, s); break;
+    }
+    if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "fma_chain launch: %s", cudaGetErrorString(e));
+    return TRI_OK;
+}
+
+}  // namespace tri
+
+extern "C" {
+
+int roofline_run_k(unsigned k, float a, float b, size_t n, const float *in, float *out, void *stream)
+{
+    return tri::run(k, a, b, n, in, out, stream);
+}
+
+int roofline_run(double ai, size_t n, const float *in, float *out, void *stream)
+{
+    if (!(ai > 0.0) || !std::isfinite(ai)) return tri::fail(TRI_ERR_INVALID_ARG, "ai must be a positive finite number");
+    double k4 = 4.0 * ai, kr = std::nearbyint(k4);
+    if (std::fabs(k4 - kr) >= 1e-9 || kr < 1.0 || kr > 1048576.0)
+        return tri::fail(TRI_ERR_INVALID_ARG, "k = 4*ai = %.12g is not an integer in [1, 2^20]", k4);
+    return tri::run((unsigned)kr, 0.9990234375f, 0.0009765625f, n, in, out, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,43 @@
+// NVML resolved at run time with dlopen("libnvidia-ml.so.1") — the build box has only the stub and the
+// compute calls must keep working where NVML is absent (include/triroof.h, TRI_ERR_NVML_UNAVAILABLE).
+// Only the handful of entry points the phase tracer and the clock-lock helpers use.
+#pragma once
+#include <cstdint>
+#include "../../include/triroof.h"
+
+namespace tri {
+namespace nvml {
+
+typedef struct nvmlDevice_st *Device;
+enum { SUCCESS = 0, ERROR_NOT_SUPPORTED = 3, ERROR_NO_PERMISSION = 4 };
+enum { CLOCK_SM = 1, CLOCK_MEM = 2 };
+enum { TEMPERATURE_GPU = 0 };
+
+struct Api {
+    bool ok = false;
+    int (*init)(void) = nullptr;
+    int (*shutdown)(void) = nullptr;
+    const char *(*error_string)(int) = nullptr;
+    int (*device_by_index)(unsigned, Device *) = nullptr;
+    int (*device_by_pci)(const char *, Device *) = nullptr;
+    int (*clock_info)(Device, int, unsigned *) = nullptr;
+    int (*temperature)(Device, int, unsigned *) = nullptr;
+    int (*power_usage)(Device, unsigned *) = nullptr;
+    int (*total_energy)(Device, unsigned long long *) = nullptr;
+    int (*clock_reasons)(Device, unsigned long long *) = nullptr;
+    int (*set_gpu_locked)(Device, unsigned, unsigned) = nullptr;
+    int (*reset_gpu_locked)(Device) = nullptr;
+    int (*set_mem_locked)(Device, unsigned, unsigned) = nullptr;
+    int (*reset_mem_locked)(Device) = nullptr;
+};
+
+// Loads and initialises NVML once per process; returns nullptr (with tri::fail text set) if unavailable.
+const Api *api();
+// NVML handle of CUDA device `device` (matched through its PCI bus id); nullptr on failure.
+Device device_handle(int device);
+void unload();
+// Fills the NVML fields of *s (t_s and phase are left to the caller).
+int read_sample(const Api *a, Device h, tri_sample *s);
+
+}  // namespace nvml
+}  // namespace tri

@@ -1,0 +1,289 @@
+// a4. Phase trace (BASELINE.json config 5; ABI in include/triroof.h).
+// A host sampler thread polls NVML (SM / memory clock, temperature, power, cumulative energy,
+// clocks-event reasons) every period into a caller-owned buffer, tagging each sample with the phase
+// current at that instant; phase_trace() is the config-5 driver that alternates the prefill GEMM, the
+// decode GEMV and an idle gap and reduces the samples to per-phase summaries.
+#include "nvml_dyn.h"
+#include "tri_internal.h"
+
+#include <time.h>
+#include <atomic>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <thread>
+#include <vector>
+
+namespace tri {
+
+static double now_s()
+{
+    timespec ts;
+    clock_gettime(CLOCK_MONOTONIC, &ts);
+    return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
+
+static void sleep_until(double t_abs)
+{
+    timespec ts;
+    ts.tv_sec = (time_t)t_abs;
+    ts.tv_nsec = (long)((t_abs - (double)ts.tv_sec) * 1e9);
+    while (clock_nanosleep(CLOCK_MONOTONIC, TIMER_ABSTIME, &ts, nullptr) != 0) {
+    }
+}
+
+struct Tracer {
+    const nvml::Api *api = nullptr;
+    nvml::Device dev = nullptr;
+    tri_sample *buf = nullptr;
+    size_t cap = 0;
+    std::atomic<size_t> n{0};
+    std::atomic<int> phase{TRI_PHASE_IDLE};
+    std::atomic<bool> stop{false};
+    bool overflow = false;
+    unsigned period_us = 10000;
+    double t0 = 0.0;
+    std::thread th;
+
+    void run()
+    {
+        double next = t0;
+        while (!stop.load(std::memory_order_acquire)) {
+            size_t i = n.load(std::memory_order_relaxed);
+            if (i >= cap) {
+                overflow = true;
+                break;
+            }
+            tri_sample s;
+            memset(&s, 0, sizeof(s));
+            nvml::read_sample(api, dev, &s);
+            s.t_s = now_s() - t0;                      // stamped after the reads: the values are at most this old
+            s.phase = phase.load(std::memory_order_acquire);
+            buf[i] = s;
+            n.store(i + 1, std::memory_order_release);
+            next += 1e-6 * period_us;
+            double t = now_s();
+            if (next < t) next = t;                    // NVML was slower than the period: do not burst
+            sleep_until(next);
+        }
+    }
+};
+
+// Reduces samples[0..ns) in [t_begin, t_end] into the clock / temperature fields of *out.
+static void reduce_window(const tri_sample *samples, size_t ns, tri_phase_summary *out)
+{
+    std::vector<const tri_sample *> w;
+    for (size_t i = 0; i < ns; ++i)
+        if (samples[i].t_s >= out->t_begin_s && samples[i].t_s <= out->t_end_s) w.push_back(&samples[i]);
+    out->n_samples = (uint32_t)w.size();
+    if (w.empty()) return;
+    double sum = 0.0, tmax = 0.0;
+    for (auto *s : w) {
+        sum += s->sm_mhz;
+        if (s->temp_c > tmax) tmax = s->temp_c;
+    }
+    out->sm_mhz_mean = (float)(sum / (double)w.size());
+    out->temp_c_max = (float)tmax;
+    size_t d = w.size() / 10;
+    if (d == 0) d = 1;
+    double f = 0.0, l = 0.0;
+    for (size_t i = 0; i < d; ++i) {
+        f += w[i]->sm_mhz;
+        l += w[w.size() - 1 - i]->sm_mhz;
+    }
+    out->sm_mhz_first10 = (float)(f / (double)d);
+    out->sm_mhz_last10 = (float)(l / (double)d);
+}
+
+static uint64_t energy_now_mj(const nvml::Api *a, nvml::Device h)
+{
+    unsigned long long e = 0;
+    if (a->total_energy && a->total_energy(h, &e) == nvml::SUCCESS) return e;
+    return 0;
+}
+
+}  // namespace tri
+
+extern "C" {
+
+int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t cap, void **handle)
+{
+    if (!buf || !handle || cap == 0) return tri::fail(TRI_ERR_INVALID_ARG, "buf/handle is NULL or cap is 0");
+    if (period_us < 1000) return tri::fail(TRI_ERR_INVALID_ARG, "period_us = %u below 1000", period_us);
+    const tri::nvml::Api *a = tri::nvml::api();
+    if (!a) return TRI_ERR_NVML_UNAVAILABLE;
+    tri::nvml::Device h = tri::nvml::device_handle(device);
+    if (!h) return TRI_ERR_NVML_UNAVAILABLE;
+    tri::Tracer *t = new (std::nothrow) tri::Tracer();
+    if (!t) return tri::fail(TRI_ERR_INVALID_ARG, "out of host memory");
+    t->api = a;
+    t->dev = h;
+    t->buf = buf;
+    t->cap = cap;
+    t->period_us = period_us;
+    t->t0 = tri::now_s();
+    t->th = std::thread([t] { t->run(); });
+    *handle = t;
+    return TRI_OK;
+}
+
+int phase_trace_mark(void *handle, int phase)
+{
+    if (!handle) return tri::fail(TRI_ERR_INVALID_ARG, "handle is NULL");
+    static_cast<tri::Tracer *>(handle)->phase.store(phase, std::memory_order_release);
+    return TRI_OK;
+}
+
+int phase_trace_stop(void *handle, size_t *n_samples)
+{
+    if (!handle) return tri::fail(TRI_ERR_INVALID_ARG, "handle is NULL");
+    tri::Tracer *t = static_cast<tri::Tracer *>(handle);
+    t->stop.store(true, std::memory_order_release);
+    if (t->th.joinable()) t->th.join();
+    if (n_samples) *n_samples = t->n.load();
+    bool ovf = t->overflow;
+    delete t;
+    if (ovf) return tri::fail(TRI_ERR_BUFFER_TOO_SMALL, "sample buffer full; trace truncated");
+    return TRI_OK;
+}
+
+int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, double decode_s, double idle_s,
+                unsigned period_ms, tri_sample *samples, size_t cap, size_t *n_samples, tri_phase_summary *summaries,
+                size_t scap, size_t *n_summaries)
+{
+    using namespace tri;
+    if (!wl || !samples || !summaries || !n_samples || !n_summaries) return fail(TRI_ERR_INVALID_ARG, "NULL argument");
+    if (!(total_s > 0) || prefill_s < 0 || decode_s < 0 || idle_s < 0 || prefill_s + decode_s + idle_s <= 0)
+        return fail(TRI_ERR_INVALID_ARG, "durations must be non-negative with a positive cycle and total");
+    if (period_ms < 1) return fail(TRI_ERR_INVALID_ARG, "period_ms must be >= 1");
+    if (prefill_s > 0 && (!wl->pa || !wl->pw || !wl->pc)) return fail(TRI_ERR_INVALID_ARG, "prefill buffers are NULL");
+    if (decode_s > 0 && (!wl->dx || !wl->dw_ring || wl->dw_count < 1 || !wl->dy))
+        return fail(TRI_ERR_INVALID_ARG, "decode buffers are NULL or dw_count < 1");
+    *n_samples = 0;
+    *n_summaries = 0;
+    const DeviceInfo *di = nullptr;
+    int st = ensure_init(&di);
+    if (st != TRI_OK) return st;
+    const nvml::Api *a = nvml::api();
+    if (!a) return TRI_ERR_NVML_UNAVAILABLE;
+    nvml::Device h = nvml::device_handle(di->device);
+    if (!h) return TRI_ERR_NVML_UNAVAILABLE;
+
+    cudaStream_t s = static_cast<cudaStream_t>(wl->stream);
+    cudaEvent_t e0, e1, ring[2];
+    TRI_CUDA(cudaEventCreate(&e0));
+    TRI_CUDA(cudaEventCreate(&e1));
+    TRI_CUDA(cudaEventCreateWithFlags(&ring[0], cudaEventDisableTiming));
+    TRI_CUDA(cudaEventCreateWithFlags(&ring[1], cudaEventDisableTiming));
+
+    void *handle = nullptr;
+    st = phase_trace_start(di->device, period_ms * 1000u, samples, cap, &handle);
+    if (st != TRI_OK) return st;
+    Tracer *tr = static_cast<Tracer *>(handle);
+    const double t0 = tr->t0;
+
+    const int lda = wl->pk, ldc = wl->pn, ldx = wl->dk, ldy = wl->dn;
+    const int p_ldw = wl->w_layout == TRI_W_NK ? wl->pk : wl->pn;
+    const int d_ldw = wl->w_layout == TRI_W_NK ? wl->dk : wl->dn;
+    const double p_flop = 2.0 * wl->pm * (double)wl->pn * wl->pk;
+    const double p_bytes = 2.0 * ((double)wl->pm * wl->pk + (double)wl->pk * wl->pn + (double)wl->pm * wl->pn);
+    const double d_flop = 2.0 * wl->dm * (double)wl->dn * wl->dk;
+    const double d_bytes = 2.0 * ((double)wl->dm * wl->dk + (double)wl->dk * wl->dn + (double)wl->dm * wl->dn);
+
+    int status = TRI_OK;
+    size_t nsum = 0;
+    uint64_t dcalls = 0;
+    bool truncated = false;
+    const int phases[3] = {TRI_PHASE_PREFILL, TRI_PHASE_DECODE, TRI_PHASE_IDLE};
+    const double durs[3] = {prefill_s, decode_s, idle_s};
+    while (status == TRI_OK && now_s() - t0 < total_s) {
+        for (int pi = 0; pi < 3 && status == TRI_OK; ++pi) {
+            if (durs[pi] <= 0) continue;
+            double remaining = total_s - (now_s() - t0);
+            if (remaining <= 0) break;
+            const double dur = durs[pi] < remaining ? durs[pi] : remaining;
+            const int ph = phases[pi];
+            tri_phase_summary sm;
+            memset(&sm, 0, sizeof(sm));
+            sm.phase = ph;
+            phase_trace_mark(handle, ph);
+            const uint64_t en0 = energy_now_mj(a, h);
+            const double tb = now_s();
+            sm.t_begin_s = tb - t0;
+            if (ph == TRI_PHASE_IDLE) {
+                sleep_until(tb + dur);                  // no kernels queued, context alive, host thread blocked
+            } else {
+                const unsigned depth = ph == TRI_PHASE_PREFILL ? 4u : 64u;   // launches per queue-bounding event
+                cudaEventRecord(e0, s);
+                uint64_t launches = 0;
+                unsigned slot = 0;
+                bool have[2] = {false, false};
+                while (now_s() - tb < dur) {
+                    for (unsigned q = 0; q < depth; ++q) {
+                        if (ph == TRI_PHASE_PREFILL)
+                            status = prefill_gemm(wl->pm, wl->pn, wl->pk, wl->pa, lda, wl->pw, p_ldw, wl->w_layout, wl->pc, ldc, s);
+                        else
+                            status = decode_gemv(wl->dm, wl->dn, wl->dk, wl->dx, ldx, wl->dw_ring[dcalls++ % wl->dw_count], d_ldw,
+                                                 wl->w_layout, wl->dy, ldy, s);
+                        if (status != TRI_OK) break;
+                        ++launches;
+                    }
+                    if (status != TRI_OK) break;
+                    cudaEventRecord(ring[slot], s);
+                    have[slot] = true;
+                    slot ^= 1;
+                    if (have[slot]) cudaEventSynchronize(ring[slot]);   // at most 2 * depth launches in flight
+                }
+                cudaEventRecord(e1, s);
+                cudaError_t ce = cudaEventSynchronize(e1);
+                if (ce != cudaSuccess && status == TRI_OK) status = fail(TRI_ERR_CUDA, "phase sync: %s", cudaGetErrorString(ce));
+                float ms = 0.f;
+                if (status == TRI_OK) cudaEventElapsedTime(&ms, e0, e1);
+                sm.gpu_ms = ms;
+                sm.launches = launches;
+                const double per_flop = ph == TRI_PHASE_PREFILL ? p_flop : d_flop;
+                const double per_bytes = ph == TRI_PHASE_PREFILL ? p_bytes : d_bytes;
+                sm.flop = per_flop * (double)launches;
+                sm.bytes = per_bytes * (double)launches;
+                sm.tokens = (double)(ph == TRI_PHASE_PREFILL ? wl->pm : wl->dm) * (double)launches;
+            }
+            const double te = now_s();
+            const uint64_t en1 = energy_now_mj(a, h);
+            sm.t_end_s = te - t0;
+            sm.energy_j = en1 >= en0 ? 1e-3 * (double)(en1 - en0) : 0.0;
+            if (nsum < scap) summaries[nsum++] = sm;
+            else truncated = true;
+        }
+    }
+    phase_trace_mark(handle, TRI_PHASE_IDLE);
+    size_t ns = 0;
+    int st2 = phase_trace_stop(handle, &ns);
+    *n_samples = ns;
+    for (size_t i = 0; i < nsum; ++i) {
+        tri_phase_summary *q = &summaries[i];
+        reduce_window(samples, ns, q);
+        const double dt = q->t_end_s - q->t_begin_s;
+        if (q->energy_j <= 0.0 && q->n_samples > 0) {          // no energy counter: integrate the power samples
+            double pw = 0.0;
+            uint32_t c = 0;
+            for (size_t j = 0; j < ns; ++j)
+                if (samples[j].t_s >= q->t_begin_s && samples[j].t_s <= q->t_end_s) { pw += samples[j].power_w; ++c; }
+            q->energy_j = c ? pw / c * dt : 0.0;
+        }
+        q->mean_power_w = dt > 0 ? q->energy_j / dt : 0.0;
+        q->j_per_flop = q->flop > 0 ? q->energy_j / q->flop : 0.0;
+        q->j_per_byte = q->bytes > 0 ? q->energy_j / q->bytes : 0.0;
+        q->j_per_token = q->tokens > 0 ? q->energy_j / q->tokens : 0.0;
+    }
+    *n_summaries = nsum;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaEventDestroy(ring[0]);
+    cudaEventDestroy(ring[1]);
+    if (status != TRI_OK) return status;
+    if (st2 != TRI_OK) return st2;
+    if (truncated) return fail(TRI_ERR_BUFFER_TOO_SMALL, "summary buffer full; later phases dropped");
+    return TRI_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,41 @@
+// Internal helpers shared by the library's translation units (not part of the ABI).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstddef>
+#include <cstdint>
+#include "../../include/triroof.h"
+
+namespace tri {
+
+struct DeviceInfo {
+    int device = -1;
+    int sm_count = 0;
+    size_t l2_bytes = 0;
+    int cc_major = 0, cc_minor = 0;
+    size_t smem_optin = 0;
+};
+
+// Sets the calling thread's detail text and returns `status` (so call sites can `return fail(...)`).
+int fail(int status, const char *fmt, ...) __attribute__((format(printf, 2, 3)));
+
+// Lazily initialises on the current device; returns TRI_OK or an error status.
+int ensure_init(const DeviceInfo **info);
+
+// cuTensorMapEncodeTiled resolved through cudaGetDriverEntryPoint (no -lcuda link dependency).
+// 2-D bf16 tensor: dims {inner, outer} elements, row pitch in bytes, box {box_inner, box_outer}.
+int make_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer,
+                      uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz);
+
+inline bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
+
+}  // namespace tri
+
+#define TRI_CUDA(call)                                                                         \
+    do {                                                                                       \
+        cudaError_t e__ = (call);                                                              \
+        if (e__ != cudaSuccess)                                                                \
+            return tri::fail(TRI_ERR_CUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e__),   \
+                             __FILE__, __LINE__);                                              \
+    } while (0)

@@ -1,0 +1,77 @@
+"""GPU checks of the phase tracer (NVML sampler + config-5 driver) and the clock helpers.  These are
+host-side integer / float records, so the checks are structural: ordering, tagging, accounting."""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import paper_2606_29629_b200 as tri
+from synth_inputs import normal_bf16_torch
+
+pytestmark = pytest.mark.gpu
+
+
+def test_nvml_sample_and_clock_probe():
+    s = tri.tri_nvml_sample(0)
+    assert s["phase"] == -1 and s["sm_mhz"] > 0 and s["mem_mhz"] > 0 and 0 < s["temp_c"] < 110 and s["power_w"] > 0
+    mhz = tri.tri_sm_clock_mhz(3000)
+    assert 100.0 < mhz < 3000.0
+
+
+def test_sampler_start_mark_stop():
+    tr = tri.PhaseTracer(0, period_us=5000, capacity=4096).start(tri.TRI_PHASE_IDLE)
+    time.sleep(0.15)
+    tr.mark(tri.TRI_PHASE_ROOFLINE)
+    x = torch.zeros(1 << 24, device="cuda")
+    for _ in range(50):
+        tri.roofline_run(16.0, x.numel(), x, x)
+    torch.cuda.synchronize()
+    time.sleep(0.05)
+    samples = tr.stop()
+    assert len(samples) >= 10
+    t = [s["t_s"] for s in samples]
+    assert all(b > a for a, b in zip(t, t[1:]))
+    phases = [s["phase"] for s in samples]
+    assert phases[0] == tri.TRI_PHASE_IDLE and phases[-1] == tri.TRI_PHASE_ROOFLINE
+    e = [s["energy_mj"] for s in samples]
+    assert all(b >= a for a, b in zip(e, e[1:]))
+
+
+def test_capacity_overflow_is_reported():
+    tr = tri.PhaseTracer(0, period_us=1000, capacity=8).start()
+    time.sleep(0.1)
+    assert len(tr.stop()) == 8
+
+
+def test_phase_trace_driver_short():
+    # a 2.0 s miniature of config 5: [0.4 s prefill | 0.4 s decode | 0.2 s idle] x 2, 10 ms sampling
+    pm, pn, pk = 1024, 4096, 1024
+    dm, dn, dk = 8, 18944, 3584
+    pa = normal_bf16_torch(4, (pm, pk), 1.0, "cuda", stream=0)
+    pw = normal_bf16_torch(4, (pn, pk), 0.02, "cuda", stream=1)
+    pc = torch.empty((pm, pn), dtype=torch.bfloat16, device="cuda")
+    dx = normal_bf16_torch(4, (dm, dk), 1.0, "cuda", stream=2)
+    dws = [normal_bf16_torch(4, (dn, dk), 0.02, "cuda", stream=3 + r) for r in range(2)]
+    dy = torch.empty((dm, dn), dtype=torch.bfloat16, device="cuda")
+    samples, summ = tri.phase_trace(pm, pn, pk, pa, pw, pc, dm, dn, dk, dx, dws, dy, tri.TRI_W_NK, total_s=2.0,
+                                    prefill_s=0.4, decode_s=0.4, idle_s=0.2, period_ms=10)
+    assert [s["phase_name"] for s in summ] == ["prefill", "decode", "idle"] * 2
+    assert 150 <= len(samples) <= 230
+    for s in summ:
+        assert s["t_end_s"] > s["t_begin_s"]
+        if s["phase_name"] == "idle":
+            assert s["launches"] == 0 and s["flop"] == 0
+            assert abs((s["t_end_s"] - s["t_begin_s"]) - 0.2) < 0.05
+        else:
+            assert s["launches"] > 10 and s["gpu_ms"] > 300
+            assert s["energy_j"] > 0 and s["j_per_flop"] > 0 and s["j_per_token"] > 0
+            assert s["n_samples"] >= 25 and s["sm_mhz_mean"] > 0
+            per = 2.0 * (pm * pn * pk if s["phase_name"] == "prefill" else dm * dn * dk)
+            assert abs(s["flop"] - per * s["launches"]) < 1e-3 * s["flop"]
+    # the sampler tagged samples with the phase the driver was in
+    tags = {s["phase"] for s in samples}
+    assert {tri.TRI_PHASE_PREFILL, tri.TRI_PHASE_DECODE, tri.TRI_PHASE_IDLE} <= tags
+    # and the GEMM output of the last prefill call is the real product (spot check)
+    ref = pa[:64].float() @ pw.float().T
+    assert (pc[:64].float() - ref).abs().max().item() < 0.05
