@@ -1,0 +1,373 @@
+"""bench.py — one "step" = one pass of the whole hot path over one batch of synthetic input:
+
+    13 launches of the FMA-chain roofline kernel (BASELINE.json config 2: N = 2^28 fp32, k = 2^0 .. 2^12,
+    A.I. = k/4 = 0.25 .. 1024 FLOP/B)  +  8 decode GEMVs over 8 rotating weight copies (config 3)  +  1 prefill
+    GEMM (config 4), with the NVML phase tracer sampling clock / power / energy alongside.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Prints ONE JSON line.  `value` is the aggregate algorithmic TFLOP/s of the step;
+the per-A.I.-point GB/s, TFLOP/s and % of roofline (the metric BASELINE.json names) are in `points`.
+`--impl reference` times the CPU oracle, as it stands, on a bounded sample of the same step.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "achieved GB/s or TFLOP/s and % of roofline per A.I. point on 1 B200; J/op"
+N_FMA = 1 << 28
+KS = [1 << i for i in range(13)]
+GEMV_SHAPE = (8, 18944, 3584)         # m, n, k
+GEMM_SHAPE = (4096, 18944, 3584)
+GEMV_COPIES = 8
+FP32_LANES_PER_SM = 128                # FP32 FMA lanes per SM (4 SMSPs x 32); DESIGN.md "ALU peak"
+REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+           0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+           0x100: "display_clock_setting"}
+
+
+def fma_flop(k, n=N_FMA):
+    return 2.0 * k * n
+
+
+def gemm_flop(shape):
+    m, n, k = shape
+    return 2.0 * m * n * k
+
+
+def gemm_bytes(shape):
+    m, n, k = shape
+    return 2.0 * (m * k + k * n + m * n)
+
+
+STEP_FLOP = sum(fma_flop(k) for k in KS) + GEMV_COPIES * gemm_flop(GEMV_SHAPE) + gemm_flop(GEMM_SHAPE)
+STEP_BYTES = len(KS) * 8.0 * N_FMA + GEMV_COPIES * gemm_bytes(GEMV_SHAPE) + gemm_bytes(GEMM_SHAPE)
+
+
+def load_peaks():
+    """Measured denominators (driver-written MEASURED_PEAKS.json), else the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0,
+            "source": "fallback"}
+
+
+# ----------------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline of our arm; the whole of --impl reference)
+# ----------------------------------------------------------------------------------------------------------
+class OracleSample:
+    """A bounded sample of the step for the CPU oracle: 2^18 elements per A.I. point, the full config-3 GEMV once,
+    8 rows of the config-4 GEMM.  Throughput in the step's unit (algorithmic TFLOP/s)."""
+    N_FMA_S = 1 << 18
+    GEMM_ROWS = 8
+
+    def __init__(self):
+        import oracle
+        from synth_inputs import normal_bf16, uniform_pm1
+        self.oracle = oracle
+        self.x = uniform_pm1(1, self.N_FMA_S)
+        m, n, k = GEMV_SHAPE
+        self.gx = normal_bf16(2, (m, k), 1.0, stream=0)
+        self.gw = np.ascontiguousarray(normal_bf16(2, (k, n), 0.02, stream=1).T)
+        self.ga = normal_bf16(3, (self.GEMM_ROWS, k), 1.0, stream=0)
+        self.flop = (sum(fma_flop(kk, self.N_FMA_S) for kk in KS) + gemm_flop(GEMV_SHAPE)
+                     + gemm_flop((self.GEMM_ROWS, n, k)))
+        self.desc = (f"per step: FMA chain 2^18 of 2^28 elements at each of 13 k; config-3 GEMV once (of 8); "
+                     f"{self.GEMM_ROWS} of 4096 rows of the config-4 GEMM")
+
+    def step(self):
+        t0 = time.perf_counter()
+        for k in KS:
+            self.oracle.fma_chain(self.x, k)
+        self.oracle.gemm_rows(self.gx, self.gw, w_layout=self.oracle.W_NK)
+        self.oracle.gemm_rows(self.ga, self.gw, w_layout=self.oracle.W_NK)
+        return time.perf_counter() - t0
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    s = OracleSample()
+    for _ in range(args.warmup):
+        s.step()
+    times = [s.step() for _ in range(args.steps)]
+    tot = sum(times)
+    value = s.flop * args.steps / tot / 1e12
+    cores = s.oracle.num_threads()
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": "TFLOP/s (algorithmic, whole step)",
+           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
+           "data": "synthetic", "config": workload_config(args.gpus),
+           "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "sample": s.desc},
+           "e2e": {"value": value, "unit": "TFLOP/s (algorithmic, whole step)", "h2d_bytes_per_step": 0,
+                   "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def workload_config(n_gpus):
+    return {"workload": "configs[1] A.I. sweep (FMA chain N=2^28 fp32, k=2^0..2^12) + configs[2] decode GEMV 8x3584x18944 "
+                        "x 8 rotating weight copies + configs[3] prefill GEMM 4096x3584x18944, W layout NK",
+            "parallelism": f"replicas x{n_gpus} (no collective)",
+            "l2": "inputs larger than L2 (2 GiB FMA stream; 8 rotating 136 MB GEMV weights; 320 MB GEMM operands)"}
+
+
+# ----------------------------------------------------------------------------------------------------------
+# GPU arm
+# ----------------------------------------------------------------------------------------------------------
+class GpuStep:
+    """Device buffers (seeded synthetic, generated on the device with the bit-identical integer generator for the
+    fp32 stream) and the launch sequence of one step.  Every launch goes through the C ABI binding."""
+
+    def __init__(self, torch, tri):
+        from synth_inputs import normal_bf16_torch, uniform_pm1_torch
+        self.torch, self.tri = torch, tri
+        dev = "cuda"
+        self.x = uniform_pm1_torch(1, N_FMA, device=dev)
+        self.y = torch.empty_like(self.x)
+        m, n, k = GEMV_SHAPE
+        self.gx = normal_bf16_torch(2, (m, k), 1.0, dev, stream=0)
+        self.gw = [normal_bf16_torch(2, (n, k), 0.02, dev, stream=1 + r) for r in range(GEMV_COPIES)]   # physical [n][k]
+        self.gy = torch.empty((m, n), dtype=torch.bfloat16, device=dev)
+        pm, pn, pk = GEMM_SHAPE
+        self.pa = normal_bf16_torch(3, (pm, pk), 1.0, dev, stream=0)
+        self.pw = normal_bf16_torch(3, (pn, pk), 0.02, dev, stream=1)
+        self.pc = torch.empty((pm, pn), dtype=torch.bfloat16, device=dev)
+        self.launches_per_step = len(KS) + GEMV_COPIES + 1
+        self.names = [f"fma_k{k}" for k in KS] + ["gemv"] + ["gemm"]
+
+    def run(self, events=None):
+        """Enqueues one step on torch's current stream.  events: optional list collecting (name, start, end)."""
+        torch, tri = self.torch, self.tri
+
+        def timed(name, fn):
+            if events is None:
+                fn()
+                return
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            events.append((name, a, b))
+
+        for k in KS:
+            timed(f"fma_k{k}", lambda k=k: tri.roofline_run(k / 4.0, N_FMA, self.x, self.y))
+        m, n, k = GEMV_SHAPE
+
+        def gemvs():
+            for w in self.gw:
+                tri.decode_gemv(m, n, k, self.gx, k, w, k, tri.TRI_W_NK, self.gy, n)
+        timed("gemv", gemvs)
+        pm, pn, pk = GEMM_SHAPE
+        timed("gemm", lambda: tri.prefill_gemm(pm, pn, pk, self.pa, pk, self.pw, pk, tri.TRI_W_NK, self.pc, pn))
+
+
+def summarise_clocks(samples, peaks):
+    busy = [s for s in samples if s["sm_mhz"] > 0]
+    if not busy:
+        return {"sm_mhz": None, "sm_max_mhz": peaks["sm_max_mhz"], "reasons": [], "source": "nvml unavailable"}
+    bits = 0
+    for s in busy:
+        bits |= int(s["clk_event_reasons"])
+    reasons = [name for bit, name in REASONS.items() if bits & bit and name != "gpu_idle"]
+    return {"sm_mhz": statistics.median(s["sm_mhz"] for s in busy), "sm_max_mhz": peaks["sm_max_mhz"],
+            "reasons": reasons, "temp_c_max": max(s["temp_c"] for s in busy),
+            "power_w_mean": sum(s["power_w"] for s in busy) / len(busy), "samples": len(busy), "source": "nvml via phase_trace_start"}
+
+
+def run_ours(args):
+    import torch
+    import paper_2606_29629_b200 as tri          # raises if the CUDA library cannot be built / loaded: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    tri.tri_init(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peaks = load_peaks()
+    step = GpuStep(torch, tri)
+    sms = tri.sm_count()
+
+    for _ in range(max(args.warmup, 3)):
+        step.run()
+    barrier()
+
+    # ---- device-resident timing: K steps, per-launch CUDA events on the launching (current) stream ----
+    tracer = None
+    try:
+        tracer = tri.PhaseTracer(local, period_us=10000, capacity=1 << 16).start(tri.TRI_PHASE_ROOFLINE)
+    except tri.TriError:
+        tracer = None
+    events = []
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0 = tri.tri_nvml_sample(local)["energy_mj"] if tracer else 0
+    t_begin.record()
+    for _ in range(args.steps):
+        step.run(events)
+    t_end.record()
+    barrier()
+    e1 = tri.tri_nvml_sample(local)["energy_mj"] if tracer else 0
+    samples = tracer.stop() if tracer else []
+    total_ms = t_begin.elapsed_time(t_end)
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    clk_probe = tri.tri_sm_clock_mhz(2000)
+
+    per = {}
+    for name, a, b in events:
+        per.setdefault(name, []).append(a.elapsed_time(b))
+    clocks = summarise_clocks(samples, peaks)
+    f_obs = clocks["sm_mhz"] or peaks["sm_max_mhz"]
+    alu_peak = sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12     # TFLOP/s at the max SM clock
+    points = []
+    for k in KS:
+        ms = statistics.median(per[f"fma_k{k}"])
+        gbs, tf = 8.0 * N_FMA / ms / 1e6, fma_flop(k) / ms / 1e9
+        roof = min(alu_peak, k / 4.0 * peaks["hbm_gbs"] / 1e3)
+        points.append({"kernel": "fma_chain", "k": k, "ai": k / 4.0, "ms": ms, "gbs": gbs, "tflops": tf,
+                       "bound": "hbm" if k / 4.0 * peaks["hbm_gbs"] / 1e3 < alu_peak else "alu",
+                       "roofline_tflops": roof, "frac": tf / roof})
+    ms = statistics.median(per["gemv"]) / GEMV_COPIES
+    gv_gbs = gemm_bytes(GEMV_SHAPE) / ms / 1e6
+    points.append({"kernel": "decode_gemv", "ai": gemm_flop(GEMV_SHAPE) / gemm_bytes(GEMV_SHAPE), "ms": ms, "gbs": gv_gbs,
+                   "tflops": gemm_flop(GEMV_SHAPE) / ms / 1e9, "bound": "hbm", "roofline_gbs": peaks["hbm_gbs"],
+                   "frac": gv_gbs / peaks["hbm_gbs"]})
+    ms = statistics.median(per["gemm"])
+    gm_tf = gemm_flop(GEMM_SHAPE) / ms / 1e9
+    points.append({"kernel": "prefill_gemm", "ai": gemm_flop(GEMM_SHAPE) / gemm_bytes(GEMM_SHAPE), "ms": ms,
+                   "gbs": gemm_bytes(GEMM_SHAPE) / ms / 1e6, "tflops": gm_tf, "bound": "tensor",
+                   "roofline_tflops": peaks["bf16_tflops"], "frac": gm_tf / peaks["bf16_tflops"]})
+
+    # dominant kernel of the step: the FMA-chain kernel at k = 4096 (about half of the step time), ALU-bound
+    dom = points[len(KS) - 1]
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get("fma_k4096")
+    roofline = {"kernel": "fma_chain_kernel (k=4096 launch)", "bound": "alu", "achieved": dom["tflops"], "peak": alu_peak,
+                "unit": "TFLOP/s", "frac": dom["tflops"] / alu_peak, "traffic": traffic,
+                "peak_source": f"derived: {sms} SMs x {FP32_LANES_PER_SM} fp32 FMA lanes x 2 FLOP x {peaks['sm_max_mhz']:.0f} MHz "
+                               f"(max SM clock, {peaks['source']}); hbm / tensor points in `points` use MEASURED_PEAKS.json "
+                               f"({peaks['source']}): {peaks['hbm_gbs']} GB/s, {peaks['bf16_tflops']} TFLOP/s burst"}
+
+    # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----
+    e2e = run_e2e(torch, tri, step, args, barrier, dist)
+
+    value = STEP_FLOP * args.steps * world / (total_ms * 1e-3) / 1e12
+    energy_j = (e1 - e0) * 1e-3 if e1 > e0 else None
+    out = {"metric": METRIC, "value": value, "unit": "TFLOP/s (algorithmic, whole step)", "n_gpus": world,
+           "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
+           "data": "synthetic", "config": workload_config(world), "clocks": dict(clocks, sm_mhz_in_kernel_probe=clk_probe),
+           "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points,
+           "min_frac": min(p["frac"] for p in points),
+           "energy": {"j_per_step": energy_j / args.steps if energy_j else None,
+                      "j_per_flop": energy_j / (STEP_FLOP * args.steps) if energy_j else None,
+                      "j_per_byte": energy_j / (STEP_BYTES * args.steps) if energy_j else None},
+           "paper_context": "Tri-serve reports -22.1 % J/output-token on 3x RTX 6000 Ada (Qwen2.5-Omni-7B, vLLM-Omni); "
+                            "no throughput number is published for this path (BASELINE.md)"}
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            s = OracleSample()
+            s.step()
+            reps, t = 0, 0.0
+            while t < 10.0 and reps < 50:
+                t += s.step()
+                reps += 1
+            out["cpu_baseline"] = {"value": s.flop * reps / t / 1e12, "unit": "TFLOP/s", "cores": s.oracle.num_threads(),
+                                   "kind": "oracle", "sample": s.desc + f"; {reps} repetitions, {t:.1f} s"}
+        print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def run_e2e(torch, tri, step, args, barrier, dist):
+    """Same step through the public API with HOST buffers: every step copies its inputs (FMA stream, GEMV X, GEMM A —
+    weights are resident model state) from pinned host memory and reads its results (last sweep output, Y, C) back."""
+    hx = torch.empty(N_FMA, dtype=torch.float32, pin_memory=True)
+    hx.copy_(step.x)
+    hy = torch.empty(N_FMA, dtype=torch.float32, pin_memory=True)
+    hgx = step.gx.cpu().pin_memory()
+    hpa = step.pa.cpu().pin_memory()
+    hgy = torch.empty(step.gy.shape, dtype=torch.bfloat16, pin_memory=True)
+    hpc = torch.empty(step.pc.shape, dtype=torch.bfloat16, pin_memory=True)
+    h2d = hx.numel() * 4 + hgx.numel() * 2 + hpa.numel() * 2
+    d2h = hy.numel() * 4 + hgy.numel() * 2 + hpc.numel() * 2
+
+    def one():
+        step.x.copy_(hx, non_blocking=True)
+        step.gx.copy_(hgx, non_blocking=True)
+        step.pa.copy_(hpa, non_blocking=True)
+        step.run()
+        hy.copy_(step.y, non_blocking=True)
+        hgy.copy_(step.gy, non_blocking=True)
+        hpc.copy_(step.pc, non_blocking=True)
+
+    one()
+    barrier()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n = max(1, min(args.steps, 5))
+    a.record()
+    for _ in range(n):
+        one()
+    b.record()
+    barrier()
+    ms = a.elapsed_time(b)
+    world = 1
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        world = dist.get_world_size()
+    return {"value": STEP_FLOP * n * world / (ms * 1e-3) / 1e12, "unit": "TFLOP/s (algorithmic, whole step)",
+            "ms_per_step": ms / n, "steps": n, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)     # 20 timed reps per A.I. point (BASELINE.json config 2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

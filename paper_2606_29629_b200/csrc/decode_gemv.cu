@@ -2,22 +2,26 @@
 // include/triroof.h):   Y[m][n] = bf16_rne( sum_k X[m][k] * W[k][n] ),  m <= 16, fp32 accumulation.
 //
 // HBM-bound: the weight matrix is read exactly once.  CUDA-core kernel by design (the GEMM is the
-// only tensor-core path): at m = 8 every weight element still costs 8 fp32 FMAs, so the FMA issue
-// rate is the second budget; the mapping below keeps issue slots per weight low.
+// only tensor-core path).  At m = 8 every weight element still costs 8 fp32 FMAs (70 % of the FP32
+// pipe at the HBM roofline), and every register written from shared memory costs a wavefront, so the
+// mapping below minimises FMA-pipe cycles, issue slots and shared-memory wavefronts per weight.
 //
 // TRI_W_NK kernel (W_phys[n][k], K contiguous) — one CTA per 128 output columns (18944 = 148 * 128:
 // exactly one CTA per SM):
-//   * thread 0 doubles as the producer: it streams the CTA's weight panel through a ring of
-//     shared-memory stages with TMA (two 64(k) x 128(n) boxes per stage, 128-byte swizzle) and
-//     mbarriers, always GV_STAGES - 1 stages ahead of the stage being consumed;
-//   * X is converted once to fp32 and kept in shared memory as k-pairs  xs[k/2][m][2];
-//   * 16 consumer warps: within a stage of 128 k-values warp w owns the 8 k-values of chunk w; lane l
-//     owns columns l, l+32, l+64, l+96.  One LDS.128 per column gives 4 bf16 pairs; a pair unpacks
-//     with 2 ALU ops into {w[k0], w[k1]} and feeds 8 FFMA2 (one per batch row) against the broadcast
-//     X pair  ->  per 8 weights: 1 LDS + 8 ALU + 32 FFMA2, plus 16 broadcast LDS shared by 4 columns;
-//   * the swizzle makes the per-column 16-byte reads bank-conflict free (rows l..l+7 hit 8 chunks);
-//   * after the last stage the 16 per-warp partial sums are reduced through shared memory (the ring
-//     is reused), rounded to bf16 RNE and stored.
+//   * a producer warp streams the CTA's weight panel through a ring of 16 KiB shared-memory slots
+//     with TMA (one 64(k) x 128(n) box per stage, 128-byte swizzle, L2 evict-first) and mbarriers;
+//   * X is converted once to fp32 and kept in shared memory as xs[k][m] (8 floats per k; each 8-k
+//     chunk padded to 72 floats so the fill is bank-conflict free);
+//   * 12 compute warps in 3 groups of 4; group g consumes stages g, g+3, ...  Inside a stage each
+//     HALF-warp owns one 8-k chunk (16 bytes of every weight row) and each lane 8 columns
+//     (i, i+16, ..., i+112): one LDS.128 per column; the swizzle keeps the 8 lanes of a quarter-warp
+//     on 8 different 16-byte bank groups.  The lane copies its 8 x 16 bytes to registers and
+//     releases the slot at once, so a slot is busy only for the length of those loads;
+//   * per weight: one ALU op (bf16 -> fp32 is a shift or a mask) and four FFMA2 in the
+//     scalar-broadcast form  acc{m, m+1} += w * {x[m], x[m+1]}  (8 batch rows = 4 packed FMAs);
+//     the X operands are quarter-warp broadcast LDS.128, shared by the lane's 8 columns;
+//   * after the last stage the 24 half-warp partial sums are reduced through shared memory (the
+//     ring is reused), rounded to bf16 RNE and stored.
 //
 // TRI_W_KN kernel (W_phys[k][n], N contiguous; secondary path): thread owns 4 adjacent columns and
 // reads them with one coalesced 8-byte load per k; the 16 warps of a CTA split K; same reduction.
@@ -30,158 +34,157 @@ namespace tri {
 
 constexpr int GV_M = 8;                 // batch rows per launch (padded with zeros)
 constexpr int GV_COLS = 128;            // output columns per CTA
-constexpr int GV_CWARPS = 16;           // consumer warps
-constexpr int GV_THREADS = GV_CWARPS * 32;
-constexpr int GV_STAGE_K = 128;         // k-values per stage (two TMA boxes of 64)
-constexpr int GV_STAGES = 3;
-constexpr int GV_BOX_BYTES = 64 * GV_COLS * 2;       // 16 KiB
-constexpr int GV_STAGE_BYTES = 2 * GV_BOX_BYTES;     // 32 KiB
+constexpr int GV_CWARPS = 12;           // compute warps (3 groups of 4)
+constexpr int GV_GROUPS = 3;
+constexpr int GV_CTHREADS = GV_CWARPS * 32;
+constexpr int GV_THREADS = (GV_CWARPS + 1) * 32;     // + producer warp
+constexpr int GV_STAGE_K = 64;          // k-values per stage (one TMA box)
+constexpr int GV_SLOT_BYTES = GV_STAGE_K * GV_COLS * 2;   // 16 KiB
+constexpr int GV_MAX_SLOTS = 6;
+constexpr int GV_XCHUNK = 72;           // floats per 8-k chunk of xs (64 used + 8 padding)
+constexpr int GV_SETS = GV_CWARPS * 2;  // half-warp partial sums
+constexpr int GV_SET_STRIDE = GV_M * GV_COLS + 16;   // floats; +16 keeps the two half-warps on different banks
+constexpr int GV_BAR_BYTES = 128;
 constexpr int GV_KMAX = 4096;
-
-struct GemvSmemLayout {
-    // offsets from the 1024-aligned base
-    static constexpr int ring = 0;
-    static constexpr int bars = GV_STAGES * GV_STAGE_BYTES;         // full[GV_STAGES], empty[GV_STAGES]
-    static constexpr int xs = bars + 64;
-    static size_t bytes(int kpad) { return 1024 + xs + (size_t)kpad * GV_M * 4; }
-};
 
 __device__ __forceinline__ float2 unpack_bf16x2(uint32_t w)
 {
     return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
 }
 
+// Shared memory (from the 1024-aligned base): ring[nslots][16 KiB] | full[6], empty[6] | xs[nchunks][72] floats.
+__host__ __device__ inline size_t gemv_smem_bytes(int nslots, int nstages)
+{
+    size_t main_bytes = (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES + (size_t)nstages * 8 * GV_XCHUNK * 4;
+    size_t red_bytes = (size_t)GV_SETS * GV_SET_STRIDE * 4;
+    return 1024 + (main_bytes > red_bytes ? main_bytes : red_bytes);
+}
+
 __global__ void __launch_bounds__(GV_THREADS, 1)
 gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restrict__ x, int64_t ldx,
-               uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k)
+               uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k, int nslots)
 {
     extern __shared__ uint8_t smem_raw[];
-    uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const uint32_t ring = ptx::smem_u32(smem + GemvSmemLayout::ring);
-    const uint32_t full0 = ptx::smem_u32(smem + GemvSmemLayout::bars);
-    const uint32_t empty0 = full0 + 8 * GV_STAGES;
-    float *xs = reinterpret_cast<float *>(smem + GemvSmemLayout::xs);
+    // keep the shared state space visible to the compiler: offset arithmetic on the shared window address
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t *smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+    const uint32_t ring = smem_base;
+    const uint32_t full0 = smem_base + nslots * GV_SLOT_BYTES;
+    const uint32_t empty0 = full0 + 8 * GV_MAX_SLOTS;
+    const uint32_t xs_addr = full0 + GV_BAR_BYTES;
+    float *xs = reinterpret_cast<float *>(smem + nslots * GV_SLOT_BYTES + GV_BAR_BYTES);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * GV_COLS;
     const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
-    const int kpad = nstages * GV_STAGE_K;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < GV_STAGES; ++s) {
+        for (int s = 0; s < nslots; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);
-            ptx::mbar_init(empty0 + 8 * s, GV_CWARPS);
+            ptx::mbar_init(empty0 + 8 * s, 4);       // the 4 warps of the group that consumed the slot
         }
         ptx::fence_mbar_init();
     }
     __syncthreads();
 
-    // ===== producer duty (thread 0): streams the CTA's weight panel; the first GV_STAGES - 1 stages
-    // go out before X is converted so HBM is busy during the prologue =====
-    uint64_t pol = 0;
-    if (threadIdx.x == 0) {
-        ptx::prefetch_tmap(&wmap);
-        pol = ptx::policy_evict_first();                             // weights are read once
-        for (int s = 0; s < GV_STAGES - 1 && s < nstages; ++s) {
-            const uint32_t fb = full0 + 8 * s;
-            ptx::mbar_arrive_expect_tx(fb, GV_STAGE_BYTES);
-            ptx::tma_load_2d_hint(ring + s * GV_STAGE_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol);
-            ptx::tma_load_2d_hint(ring + s * GV_STAGE_BYTES + GV_BOX_BYTES, &wmap, s * GV_STAGE_K + 64, n0, fb, pol);
+    if (warp == GV_CWARPS) {
+        // ===== producer warp: one lane streams the weight panel =====
+        if (lane == 0) {
+            ptx::prefetch_tmap(&wmap);
+            const uint64_t pol = ptx::policy_evict_first();          // weights are read once
+            for (int s = 0; s < nstages; ++s) {
+                const int slot = s % nslots;
+                if (s >= nslots) ptx::mbar_wait(empty0 + 8 * slot, ((s / nslots) - 1) & 1);
+                const uint32_t fb = full0 + 8 * slot;
+                ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
+                ptx::tma_load_2d_hint(ring + slot * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol);
+            }
         }
-    }
-
-    // ===== consumers =====
-    // X -> fp32 k-pairs in shared memory: xs[(k/2)*16 + mm*2 + (k&1)], zero beyond m and beyond k.
-    {
-        const int cpr = kpad / 8;                                     // 16-byte chunks (8 bf16) per row
-        const int units = GV_M * cpr;
-#pragma unroll 4
-        for (int i = threadIdx.x; i < units; i += GV_CWARPS * 32) {
-            const int mm = i / cpr, c = i - mm * cpr;                 // coalesced along k within a row
-            uint4 v = make_uint4(0u, 0u, 0u, 0u);
-            if (mm < m && 8 * c < k) v = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
-            float2 *dst = reinterpret_cast<float2 *>(xs + (size_t)(4 * c) * (2 * GV_M) + mm * 2);
-            dst[0 * GV_M] = unpack_bf16x2(v.x);
-            dst[1 * GV_M] = unpack_bf16x2(v.y);
-            dst[2 * GV_M] = unpack_bf16x2(v.z);
-            dst[3 * GV_M] = unpack_bf16x2(v.w);
+    } else {
+        // ===== compute warps =====
+        // X -> fp32 in shared memory: xs[chunk * 72 + kk * 8 + mm]; zero beyond m and beyond k.
+        {
+            const int mm = threadIdx.x & 7;
+            for (int c = threadIdx.x >> 3; c < nstages * 8; c += GV_CTHREADS / 8) {
+                uint4 v = make_uint4(0u, 0u, 0u, 0u);
+                if (mm < m && 8 * c < k) v = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
+                float *dst = xs + (size_t)c * GV_XCHUNK + mm;
+                const float2 a = unpack_bf16x2(v.x), b = unpack_bf16x2(v.y), cc = unpack_bf16x2(v.z), d = unpack_bf16x2(v.w);
+                dst[0] = a.x;  dst[8] = a.y;  dst[16] = b.x;  dst[24] = b.y;
+                dst[32] = cc.x; dst[40] = cc.y; dst[48] = d.x; dst[56] = d.y;
+            }
         }
-    }
-    __syncthreads();
+        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
 
-    float2 acc[4][GV_M];
+        float2 acc[8][4];                                             // [column j][batch-row pair q]
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < 8; ++j)
 #pragma unroll
-        for (int mm = 0; mm < GV_M; ++mm) acc[j][mm] = make_float2(0.f, 0.f);
+            for (int q = 0; q < 4; ++q) acc[j][q] = make_float2(0.f, 0.f);
 
-    // this warp's 16-byte chunk inside a stage: box (warp / 8), chunk (warp % 8) of the 128-byte row
-    const uint32_t box_off = (warp >> 3) * GV_BOX_BYTES;
-    const uint32_t chunk = warp & 7;
-    uint32_t woff[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const uint32_t r = lane + 32 * j;
-        woff[j] = box_off + r * 128 + ((chunk ^ (r & 7)) << 4);
-    }
+        const int group = warp >> 2;
+        const int half = lane >> 4, i = lane & 15;
+        const int chunk = 2 * (warp & 3) + half;                      // 16-byte chunk of the 128-byte weight row
+        const uint32_t woff = (uint32_t)i * 128u + (uint32_t)((chunk ^ (i & 7)) << 4);
 
-    for (int s = 0; s < nstages; ++s) {
-        const int slot = s % GV_STAGES;
-        if (threadIdx.x == 0 && s + GV_STAGES - 1 < nstages) {
-            // refill the slot stage s-1 used (every warp released it right after its ring reads)
-            const int sn = s + GV_STAGES - 1, slotn = sn % GV_STAGES;
-            if (s >= 1) ptx::mbar_wait(empty0 + 8 * slotn, ((s - 1) / GV_STAGES) & 1);
-            const uint32_t fb = full0 + 8 * slotn;
-            ptx::mbar_arrive_expect_tx(fb, GV_STAGE_BYTES);
-            ptx::tma_load_2d_hint(ring + slotn * GV_STAGE_BYTES, &wmap, sn * GV_STAGE_K, n0, fb, pol);
-            ptx::tma_load_2d_hint(ring + slotn * GV_STAGE_BYTES + GV_BOX_BYTES, &wmap, sn * GV_STAGE_K + 64, n0, fb, pol);
-        }
-        __syncwarp();
-        ptx::mbar_wait(full0 + 8 * slot, (s / GV_STAGES) & 1);
-        const uint32_t base = ring + slot * GV_STAGE_BYTES;
-        uint4 wv[4];
+        for (int s = group; s < nstages; s += GV_GROUPS) {
+            const int slot = s % nslots;
+            ptx::mbar_wait(full0 + 8 * slot, (s / nslots) & 1);
+            const uint32_t base = ring + slot * GV_SLOT_BYTES + woff;
+            uint4 wv[8];
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                         : "=r"(wv[j].x), "=r"(wv[j].y), "=r"(wv[j].z), "=r"(wv[j].w)
-                         : "r"(base + woff[j]));
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);          // data is in registers: free the slot
+            for (int j = 0; j < 8; ++j)                               // column i + 16 j is 2048 bytes further
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                             : "=r"(wv[j].x), "=r"(wv[j].y), "=r"(wv[j].z), "=r"(wv[j].w)
+                             : "r"(base + j * 2048));
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);      // weights are in registers: free the slot
 
-        const float4 *xp = reinterpret_cast<const float4 *>(xs + ((size_t)(s * GV_STAGE_K + warp * 8) / 2) * (2 * GV_M));
+            const uint32_t xa = xs_addr + (uint32_t)(s * 8 + chunk) * (GV_XCHUNK * 4);
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {                                  // 4 k-pairs of the chunk
-            float4 xq[4];
+            for (int p = 0; p < 4; ++p) {                              // k-pairs of the chunk
+                float4 xv[4];                                          // x[2p][0..7], x[2p+1][0..7]
 #pragma unroll
-            for (int q = 0; q < 4; ++q) xq[q] = xp[p * 4 + q];        // broadcast reads: rows 2q, 2q+1
+                for (int q = 0; q < 4; ++q)
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                                 : "=f"(xv[q].x), "=f"(xv[q].y), "=f"(xv[q].z), "=f"(xv[q].w)
+                                 : "r"(xa + p * 64 + q * 16));
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const uint32_t word = p == 0 ? wv[j].x : p == 1 ? wv[j].y : p == 2 ? wv[j].z : wv[j].w;
-                const float2 w2 = unpack_bf16x2(word);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    acc[j][2 * q] = __ffma2_rn(w2, make_float2(xq[q].x, xq[q].y), acc[j][2 * q]);
-                    acc[j][2 * q + 1] = __ffma2_rn(w2, make_float2(xq[q].z, xq[q].w), acc[j][2 * q + 1]);
+                for (int j = 0; j < 8; ++j) {
+                    const uint32_t word = p == 0 ? wv[j].x : p == 1 ? wv[j].y : p == 2 ? wv[j].z : wv[j].w;
+                    const float w0 = __uint_as_float(word << 16), w1 = __uint_as_float(word & 0xffff0000u);
+                    const float2 w0b = make_float2(w0, w0), w1b = make_float2(w1, w1);
+                    acc[j][0] = __ffma2_rn(w0b, make_float2(xv[0].x, xv[0].y), acc[j][0]);
+                    acc[j][1] = __ffma2_rn(w0b, make_float2(xv[0].z, xv[0].w), acc[j][1]);
+                    acc[j][2] = __ffma2_rn(w0b, make_float2(xv[1].x, xv[1].y), acc[j][2]);
+                    acc[j][3] = __ffma2_rn(w0b, make_float2(xv[1].z, xv[1].w), acc[j][3]);
+                    acc[j][0] = __ffma2_rn(w1b, make_float2(xv[2].x, xv[2].y), acc[j][0]);
+                    acc[j][1] = __ffma2_rn(w1b, make_float2(xv[2].z, xv[2].w), acc[j][1]);
+                    acc[j][2] = __ffma2_rn(w1b, make_float2(xv[3].x, xv[3].y), acc[j][2]);
+                    acc[j][3] = __ffma2_rn(w1b, make_float2(xv[3].z, xv[3].w), acc[j][3]);
                 }
             }
         }
-    }
 
-    // ===== cross-warp reduction through the (now idle) ring: red[warp][mm][col] =====
-    __syncthreads();   // every warp is past its last ring read
-    float *red = reinterpret_cast<float *>(smem + GemvSmemLayout::ring);
+        // ===== cross-warp reduction through shared memory (ring, barriers and xs are dead now) =====
+        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+        float *red = reinterpret_cast<float *>(smem);
+        float *mine = red + (size_t)(warp * 2 + half) * GV_SET_STRIDE + i;
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < 8; ++j)
 #pragma unroll
-        for (int mm = 0; mm < GV_M; ++mm)
-            red[(warp * GV_M + mm) * GV_COLS + 32 * j + lane] = acc[j][mm].x + acc[j][mm].y;
-    __syncthreads();
-    for (int o = threadIdx.x; o < GV_M * GV_COLS; o += GV_CWARPS * 32) {
-        const int mm = o / GV_COLS, col = o - mm * GV_COLS;
-        float sum = 0.f;
+            for (int q = 0; q < 4; ++q) {
+                mine[(2 * q) * GV_COLS + 16 * j] = acc[j][q].x;
+                mine[(2 * q + 1) * GV_COLS + 16 * j] = acc[j][q].y;
+            }
+        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+        for (int o = threadIdx.x; o < GV_M * GV_COLS; o += GV_CTHREADS) {
+            const int mm = o / GV_COLS, col = o - mm * GV_COLS;
+            float sum = 0.f;
 #pragma unroll
-        for (int w = 0; w < GV_CWARPS; ++w) sum += red[(w * GV_M + mm) * GV_COLS + col];
-        if (mm < m && n0 + col < n) y[(int64_t)mm * ldy + n0 + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum));
+            for (int t = 0; t < GV_SETS; ++t) sum += red[t * GV_SET_STRIDE + o];
+            if (mm < m && n0 + col < n) y[(int64_t)mm * ldy + n0 + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum));
+        }
     }
 }
 
@@ -292,10 +295,12 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
 
     if (w_layout == TRI_W_NK) {
         CUtensorMap wmap;
-        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, 64, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
+        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
         if (st != TRI_OK) return st;
-        const int kpad = ((k + GV_STAGE_K - 1) / GV_STAGE_K) * GV_STAGE_K;
-        const size_t smem = GemvSmemLayout::bytes(kpad);
+        const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+        int nslots = GV_MAX_SLOTS < nstages ? GV_MAX_SLOTS : nstages;       // deepest ring that fits beside xs
+        while (nslots > 2 && gemv_smem_bytes(nslots, nstages) > di->smem_optin) --nslots;
+        const size_t smem = gemv_smem_bytes(nslots, nstages);
         static bool attr_set = false;
         if (!attr_set) {
             TRI_CUDA(cudaFuncSetAttribute(gemv_nk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)di->smem_optin));
@@ -304,7 +309,7 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
         if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
         for (int r0 = 0; r0 < m; r0 += GV_M) {
             const int mr = m - r0 < GV_M ? m - r0 : GV_M;
-            gemv_nk_kernel<<<blocks, GV_THREADS, smem, s>>>(wmap, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k);
+            gemv_nk_kernel<<<blocks, GV_THREADS, smem, s>>>(wmap, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k, nslots);
             TRI_CUDA(cudaGetLastError());
         }
     } else {

@@ -7,6 +7,7 @@ import torch
 
 import oracle
 import paper_2606_29629_b200 as tri
+from tests.tolerance import stated_bound, widened_bound
 from synth_inputs import bf16_bits_to_f32, f32_to_bf16_bits, normal_bf16, normal_bf16_torch, stratified_rows
 
 pytestmark = pytest.mark.gpu
@@ -34,12 +35,14 @@ def run_gemm(a_bits, w_phys, m, n, k, layout, lda=None, ldw=None, ldc=None):
     return c[:, :n]
 
 
-def check_rows(c_bits_rows, a_bits, w_phys, layout, rows=None):
+def check_rows(c_bits_rows, a_bits, w_phys, layout, rows=None, stated=False):
+    """stated=True: the north_star bound as written (configured workload); else widened by the bf16 output
+    half-ulp where that exceeds it (tests/tolerance.py)."""
     r = oracle.gemm_rows(a_bits, w_phys, rows=rows, w_layout=layout)
     g = bf16_bits_to_f32(c_bits_rows).astype(np.float64)
     assert np.isfinite(g).all()
     err = np.abs(g - r["c64"])
-    bound = TOL * r["s64"]
+    bound = stated_bound(r["s64"]) if stated else widened_bound(r["c64"], r["s64"], a_bits.shape[1])
     worst = np.unravel_index(np.argmax(err - bound), err.shape)
     assert (err <= bound).all(), f"worst at {worst}: got {g[worst]} want {r['c64'][worst]} bound {bound[worst]:.3e}"
 
@@ -121,7 +124,7 @@ def test_config4_sampled_rows(layout):
     torch.cuda.synchronize()
     rows = stratified_rows(3, m, 64)
     c_rows = dc[torch.from_numpy(rows.astype(np.int64)).cuda()].cpu().numpy().view(np.uint16)
-    check_rows(c_rows, a, wp, layout, rows=rows)
+    check_rows(c_rows, a, wp, layout, rows=rows, stated=True)
     # every output was written (no NaN filler left) and agrees with a bf16 tensor-core product to bf16 precision
     ref = (da.view(torch.bfloat16).float()[::97] @ (dw.view(torch.bfloat16).float().T if layout == tri.TRI_W_NK
                                                      else dw.view(torch.bfloat16).float()))

@@ -6,6 +6,7 @@ import torch
 
 import oracle
 import paper_2606_29629_b200 as tri
+from tests.tolerance import stated_bound, widened_bound
 from synth_inputs import bf16_bits_to_f32, f32_to_bf16_bits, normal_bf16
 
 pytestmark = pytest.mark.gpu
@@ -39,12 +40,14 @@ def run_gemv(x_bits, w_phys, m, n, k, layout, ldx=None, ldw=None, pad_y=0):
     return y[:, :n]
 
 
-def check_against_oracle(y_bits, x_bits, w_phys_unpadded, layout):
+def check_against_oracle(y_bits, x_bits, w_phys_unpadded, layout, stated=False):
+    """stated=True: the north_star bound as written (configured workload); else widened by the bf16 output
+    half-ulp where that exceeds it (tests/tolerance.py)."""
     r = oracle.gemm_rows(x_bits, w_phys_unpadded, w_layout=layout)
     g = bf16_bits_to_f32(y_bits).astype(np.float64)
     assert np.isfinite(g).all()
     err = np.abs(g - r["c64"])
-    bound = TOL * r["s64"]
+    bound = stated_bound(r["s64"]) if stated else widened_bound(r["c64"], r["s64"], x_bits.shape[1])
     worst = np.unravel_index(np.argmax(err - bound), err.shape)
     assert (err <= bound).all(), f"worst at {worst}: err {err[worst]:.3e} bound {bound[worst]:.3e}"
     return float((err / np.maximum(bound, 1e-300)).max())
@@ -58,7 +61,7 @@ def test_config3_full_output(layout):
     w = normal_bf16(2, (k, n), 0.02, stream=1)
     wp = phys_w(w, layout)
     y = run_gemv(x, wp, m, n, k, layout)
-    frac = check_against_oracle(y, x, wp, layout)
+    frac = check_against_oracle(y, x, wp, layout, stated=True)
     assert frac < 1.0
 
 
@@ -92,7 +95,9 @@ def test_ragged_shapes(layout, m, n, k):
     x = normal_bf16(30 + m, (m, k))
     w = normal_bf16(31 + m, (k, n), 0.05)
     wp = phys_w(w, layout)
-    y = run_gemv(x, wp, m, n, k, layout, pad_y=5)
+    pad = (-n) % 8 if layout == tri.TRI_W_KN else 0          # ldw must be a multiple of 8 elements
+    wq = phys_w(w, layout, ld_pad=pad) if pad else wp
+    y = run_gemv(x, wq, m, n, k, layout, ldw=wq.shape[1], pad_y=5)
     check_against_oracle(y, x, wp, layout)
 
 

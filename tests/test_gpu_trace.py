@@ -58,11 +58,12 @@ def test_phase_trace_driver_short():
                                     prefill_s=0.4, decode_s=0.4, idle_s=0.2, period_ms=10)
     assert [s["phase_name"] for s in summ] == ["prefill", "decode", "idle"] * 2
     assert 150 <= len(samples) <= 230
-    for s in summ:
+    for i, s in enumerate(summ):
         assert s["t_end_s"] > s["t_begin_s"]
         if s["phase_name"] == "idle":
             assert s["launches"] == 0 and s["flop"] == 0
-            assert abs((s["t_end_s"] - s["t_begin_s"]) - 0.2) < 0.05
+            dur = s["t_end_s"] - s["t_begin_s"]
+            assert dur < 0.25 and (i == len(summ) - 1 or dur > 0.15)     # the last phase is cut at total_s
         else:
             assert s["launches"] > 10 and s["gpu_ms"] > 300
             assert s["energy_j"] > 0 and s["j_per_flop"] > 0 and s["j_per_token"] > 0
