@@ -78,6 +78,10 @@ gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restr
     const int n0 = blockIdx.x * GV_COLS;
     const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
 
+    // Programmatic dependent launch: let the next kernel of the stream start on SMs as they drain.  The
+    // weight stream (model state, never an output of the preceding kernel) is prefetched at once; X and
+    // Y are touched only after pdl_wait(), i.e. after the preceding grid has completed.
+    ptx::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < nslots; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);
@@ -92,26 +96,51 @@ gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restr
         if (lane == 0) {
             ptx::prefetch_tmap(&wmap);
             const uint64_t pol = ptx::policy_evict_first();          // weights are read once
+            int slot = 0;
+            uint32_t par = 1;                                        // parity of the slot's previous release
             for (int s = 0; s < nstages; ++s) {
-                const int slot = s % nslots;
-                if (s >= nslots) ptx::mbar_wait(empty0 + 8 * slot, ((s / nslots) - 1) & 1);
+                if (s >= nslots) ptx::mbar_wait(empty0 + 8 * slot, par);
                 const uint32_t fb = full0 + 8 * slot;
                 ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
                 ptx::tma_load_2d_hint(ring + slot * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol);
+                if (++slot == nslots) { slot = 0; par ^= 1; }
             }
         }
     } else {
         // ===== compute warps =====
         // X -> fp32 in shared memory: xs[chunk * 72 + kk * 8 + mm]; zero beyond m and beyond k.
+        ptx::pdl_wait();
+        // A thread takes one 8-k chunk of FOUR batch rows: 4 x 16-byte loads (all issued before the first store:
+        // they are L2 hits of ~1 us latency), then 8 x 16-byte stores {x[m0..m0+3][kk]} — conflict free because
+        // consecutive chunks are 72 floats apart.
         {
-            const int mm = threadIdx.x & 7;
-            for (int c = threadIdx.x >> 3; c < nstages * 8; c += GV_CTHREADS / 8) {
-                uint4 v = make_uint4(0u, 0u, 0u, 0u);
-                if (mm < m && 8 * c < k) v = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
-                float *dst = xs + (size_t)c * GV_XCHUNK + mm;
-                const float2 a = unpack_bf16x2(v.x), b = unpack_bf16x2(v.y), cc = unpack_bf16x2(v.z), d = unpack_bf16x2(v.w);
-                dst[0] = a.x;  dst[8] = a.y;  dst[16] = b.x;  dst[24] = b.y;
-                dst[32] = cc.x; dst[40] = cc.y; dst[48] = d.x; dst[56] = d.y;
+            const int mh = threadIdx.x & 1, nchunks = nstages * 8;
+            constexpr int CSTEP = GV_CTHREADS / 2, XB = 3;            // 192 chunks per pass
+            for (int cb = threadIdx.x >> 1; cb < nchunks; cb += CSTEP * XB) {
+                uint4 v[XB][4];
+#pragma unroll
+                for (int u = 0; u < XB; ++u)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const int c = cb + u * CSTEP, mm = mh * 4 + r;
+                        v[u][r] = make_uint4(0u, 0u, 0u, 0u);
+                        if (mm < m && 8 * c < k) v[u][r] = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
+                    }
+#pragma unroll
+                for (int u = 0; u < XB; ++u) {
+                    const int c = cb + u * CSTEP;
+                    if (c < nchunks) {
+                        float4 *dst = reinterpret_cast<float4 *>(xs + (size_t)c * GV_XCHUNK + mh * 4);
+                        const uint32_t *w0 = &v[u][0].x, *w1 = &v[u][1].x, *w2 = &v[u][2].x, *w3 = &v[u][3].x;
+#pragma unroll
+                        for (int pp = 0; pp < 4; ++pp) {              // bf16 pair pp = k-values 2pp, 2pp+1
+                            const float2 a = unpack_bf16x2(w0[pp]), b = unpack_bf16x2(w1[pp]), cc = unpack_bf16x2(w2[pp]),
+                                         d = unpack_bf16x2(w3[pp]);
+                            dst[(2 * pp) * 2] = make_float4(a.x, b.x, cc.x, d.x);        // 8 floats (2 float4) per k
+                            dst[(2 * pp + 1) * 2] = make_float4(a.y, b.y, cc.y, d.y);
+                        }
+                    }
+                }
             }
         }
         asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
@@ -127,9 +156,10 @@ gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restr
         const int chunk = 2 * (warp & 3) + half;                      // 16-byte chunk of the 128-byte weight row
         const uint32_t woff = (uint32_t)i * 128u + (uint32_t)((chunk ^ (i & 7)) << 4);
 
+        int slot = group % nslots;
+        uint32_t par = (uint32_t)(group / nslots) & 1;
         for (int s = group; s < nstages; s += GV_GROUPS) {
-            const int slot = s % nslots;
-            ptx::mbar_wait(full0 + 8 * slot, (s / nslots) & 1);
+            ptx::mbar_wait(full0 + 8 * slot, par);
             const uint32_t base = ring + slot * GV_SLOT_BYTES + woff;
             uint4 wv[8];
 #pragma unroll
@@ -152,7 +182,8 @@ gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restr
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const uint32_t word = p == 0 ? wv[j].x : p == 1 ? wv[j].y : p == 2 ? wv[j].z : wv[j].w;
-                    const float w0 = __uint_as_float(word << 16), w1 = __uint_as_float(word & 0xffff0000u);
+                    // PRMT / LOP3 (ALU pipe): a shift would be turned into an IMAD on the FMA pipe, which is the busy one
+                    const float w0 = __uint_as_float(__byte_perm(word, 0u, 0x1044)), w1 = __uint_as_float(word & 0xffff0000u);
                     const float2 w0b = make_float2(w0, w0), w1b = make_float2(w1, w1);
                     acc[j][0] = __ffma2_rn(w0b, make_float2(xv[0].x, xv[0].y), acc[j][0]);
                     acc[j][1] = __ffma2_rn(w0b, make_float2(xv[0].z, xv[0].w), acc[j][1]);
@@ -164,26 +195,34 @@ gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restr
                     acc[j][3] = __ffma2_rn(w1b, make_float2(xv[3].z, xv[3].w), acc[j][3]);
                 }
             }
+#pragma unroll
+            for (int t = 0; t < GV_GROUPS; ++t)                        // advance GV_GROUPS stages round the ring
+                if (++slot == nslots) { slot = 0; par ^= 1; }
         }
 
         // ===== cross-warp reduction through shared memory (ring, barriers and xs are dead now) =====
         asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-        float *red = reinterpret_cast<float *>(smem);
-        float *mine = red + (size_t)(warp * 2 + half) * GV_SET_STRIDE + i;
+        // red[set][(j * 4 + q) * 32 + i * 2 + e] holds the partial sum of column i + 16 j, batch row 2 q + e.
+        float2 *red = reinterpret_cast<float2 *>(smem);
+        float2 *mine = red + (size_t)(warp * 2 + half) * (GV_SET_STRIDE / 2) + i;
 #pragma unroll
         for (int j = 0; j < 8; ++j)
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                mine[(2 * q) * GV_COLS + 16 * j] = acc[j][q].x;
-                mine[(2 * q + 1) * GV_COLS + 16 * j] = acc[j][q].y;
-            }
+            for (int q = 0; q < 4; ++q) mine[(j * 4 + q) * 16] = acc[j][q];
         asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-        for (int o = threadIdx.x; o < GV_M * GV_COLS; o += GV_CTHREADS) {
-            const int mm = o / GV_COLS, col = o - mm * GV_COLS;
-            float sum = 0.f;
+        for (int o = threadIdx.x; o < GV_M * GV_COLS / 2; o += GV_CTHREADS) {
+            float2 sum = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int t = 0; t < GV_SETS; ++t) sum += red[t * GV_SET_STRIDE + o];
-            if (mm < m && n0 + col < n) y[(int64_t)mm * ldy + n0 + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum));
+            for (int t = 0; t < GV_SETS; ++t) {
+                const float2 v = red[t * (GV_SET_STRIDE / 2) + o];
+                sum.x += v.x;
+                sum.y += v.y;
+            }
+            const int ii = o & 15, q = (o >> 4) & 3, j = o >> 6, col = n0 + ii + 16 * j;
+            if (col < n) {
+                if (2 * q < m) y[(int64_t)(2 * q) * ldy + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum.x));
+                if (2 * q + 1 < m) y[(int64_t)(2 * q + 1) * ldy + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum.y));
+            }
         }
     }
 }
@@ -309,8 +348,18 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
         if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
         for (int r0 = 0; r0 < m; r0 += GV_M) {
             const int mr = m - r0 < GV_M ? m - r0 : GV_M;
-            gemv_nk_kernel<<<blocks, GV_THREADS, smem, s>>>(wmap, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k, nslots);
-            TRI_CUDA(cudaGetLastError());
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(blocks);
+            cfg.blockDim = dim3(GV_THREADS);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = s;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = 1;
+            TRI_CUDA(cudaLaunchKernelEx(&cfg, gemv_nk_kernel, wmap, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k,
+                                        nslots));
         }
     } else {
         const size_t smem = ((size_t)k * GV_M + (size_t)KN_WARPS * GV_M * GV_COLS) * 4;

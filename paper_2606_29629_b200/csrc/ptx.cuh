@@ -104,6 +104,13 @@ __device__ __forceinline__ uint64_t policy_evict_last()
     return p;
 }
 
+// ---- programmatic dependent launch ----------------------------------------------------------------
+// launch_dependents: the next kernel in the stream (if launched with programmatic stream serialization)
+// may start its CTAs as soon as this grid's CTAs have all issued this or exited.
+// wait: blocks until the preceding grid has completed and its memory is visible.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // ---- tcgen05 / TMEM -----------------------------------------------------------------------------
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols)   // one full warp
 {
