@@ -101,6 +101,10 @@ int roofline_run_k(unsigned k, float a, float b, size_t n, const float *in, floa
  * w: device, bf16, layout w_layout (TRI_W_NK: ldw >= k; TRI_W_KN: ldw >= n), ldw % 8 == 0.
  * y: device, bf16 Y[i * ldy + j], ldy >= n.  x, w 16-byte aligned; y 2-byte aligned (any ldy).
  * Outputs must not alias inputs.  Asynchronous: one kernel per 8 rows of X on `stream`.
+ * The kernel is launched with programmatic stream serialization: it prefetches W (model state) while
+ * the kernel before it on `stream` drains, and reads X / writes Y only after that kernel has completed.
+ * W must therefore not be an output of the immediately preceding decode_gemv call on the same stream
+ * (any other producer of W is ordered as usual).
  */
 int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw,
                 int w_layout, uint16_t *y, int64_t ldy, void *stream);
