@@ -68,6 +68,24 @@ def load_peaks():
             "source": "fallback"}
 
 
+def ncu_traffic_bytes(kernel, column):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed text summary of the ncu
+    --set full capture (profiles/<round>_ncu_<kernel>.txt, newest round); None when there is no summary."""
+    import glob
+    import re
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"*_ncu_{kernel}.txt")))
+    if not files:
+        return None
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    total = 0.0
+    for name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(r"^%s \[(\w+)\]: (.*)$" % re.escape(name), open(files[-1]).read(), re.M)
+        if not m:
+            return None
+        total += float(m.group(2).split("|")[column].strip().replace(",", "")) * scale[m.group(1)]
+    return total
+
+
 # ----------------------------------------------------------------------------------------------------------
 # CPU oracle leg (cpu_baseline of our arm; the whole of --impl reference)
 # ----------------------------------------------------------------------------------------------------------
@@ -272,10 +290,7 @@ def run_ours(args):
 
     # dominant kernel of the step: the FMA-chain kernel at k = 4096 (about half of the step time), ALU-bound
     dom = points[len(KS) - 1]
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("fma_k4096")
+    traffic = ncu_traffic_bytes("fma_chain", column=len(KS) - 1)
     roofline = {"kernel": "fma_chain_kernel (k=4096 launch)", "bound": "alu", "achieved": dom["tflops"], "peak": alu_peak,
                 "unit": "TFLOP/s", "frac": dom["tflops"] / alu_peak, "traffic": traffic,
                 "peak_source": f"derived: {sms} SMs x {FP32_LANES_PER_SM} fp32 FMA lanes x 2 FLOP x {peaks['sm_max_mhz']:.0f} MHz "
