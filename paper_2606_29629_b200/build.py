@@ -13,7 +13,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["core.cu", "fma_chain.cu", "decode_gemv.cu", "prefill_gemm.cu", "nvml_dyn.cu", "phase_trace.cu"]
+SOURCES = ["core.cu", "fma_chain.cu", "decode_gemv.cu", "decode_gemv_m8.cu", "prefill_gemm.cu", "nvml_dyn.cu", "phase_trace.cu"]
 HEADERS = ["tri_internal.h", "ptx.cuh", "nvml_dyn.h", os.path.join("..", "..", "include", "triroof.h")]
 LIB = os.path.join(HERE, "libtriroof.so")
 OBJDIR = os.path.join(HERE, "build")
@@ -46,7 +46,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(OBJDIR, os.path.basename(src) + ".o")
         objs.append(obj)
         if force or _stale(obj, [src] + hdrs + [os.path.abspath(__file__)]):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            extra = os.environ.get("TRI_NVCC_EXTRA", "").split()          # debug only (e.g. -DSOME_EXPERIMENT)
+            cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
             procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for cmd, p in procs:
         out, _ = p.communicate()

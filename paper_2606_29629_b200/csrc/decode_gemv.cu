@@ -2,308 +2,301 @@
 // include/triroof.h):   Y[m][n] = bf16_rne( sum_k X[m][k] * W[k][n] ),  m <= 16, fp32 accumulation.
 //
 // HBM-bound: the weight matrix is read exactly once.  CUDA-core kernel by design (the GEMM is the
-// only tensor-core path).  At m = 8 every weight element still costs 8 fp32 FMAs (70 % of the FP32
-// pipe at the HBM roofline), and every register written from shared memory costs a wavefront, so the
-// mapping below minimises FMA-pipe cycles, issue slots and shared-memory wavefronts per weight.
+// only tensor-core path).  The arithmetic is the sm_100 mixed-precision FMA  fma.rn.f32.bf16
+// (SASS FHFMA.BF16): d = a * b + c with a, b bf16 taken from either half of a 32-bit register and c, d
+// fp32, one rounding — bit-identical to fmaf on the widened inputs, at the full FP32 rate (measured:
+// 125 of 128 lanes/clk/SM) and with no unpack instruction at all.  So the packed bf16 words of W and X
+// go from shared memory straight into the FMA, and a weight costs m FMA-pipe slots.
 //
-// TRI_W_NK kernel (W_phys[n][k], K contiguous) — one CTA per 128 output columns (18944 = 148 * 128:
-// exactly one CTA per SM):
-//   * a producer warp streams the CTA's weight panel through a ring of 16 KiB shared-memory slots
-//     with TMA (one 64(k) x 128(n) box per stage, 128-byte swizzle, L2 evict-first) and mbarriers;
-//   * X is converted once to fp32 and kept in shared memory as xs[k][m] (8 floats per k; each 8-k
-//     chunk padded to 72 floats so the fill is bank-conflict free);
-//   * 12 compute warps in 3 groups of 4; group g consumes stages g, g+3, ...  Inside a stage each
-//     HALF-warp owns one 8-k chunk (16 bytes of every weight row) and each lane 8 columns
-//     (i, i+16, ..., i+112): one LDS.128 per column; the swizzle keeps the 8 lanes of a quarter-warp
-//     on 8 different 16-byte bank groups.  The lane copies its 8 x 16 bytes to registers and
-//     releases the slot at once, so a slot is busy only for the length of those loads;
-//   * per weight: one ALU op (bf16 -> fp32 is a shift or a mask) and four FFMA2 in the
-//     scalar-broadcast form  acc{m, m+1} += w * {x[m], x[m+1]}  (8 batch rows = 4 packed FMAs);
-//     the X operands are quarter-warp broadcast LDS.128, shared by the lane's 8 columns;
-//   * after the last stage the 24 half-warp partial sums are reduced through shared memory (the
-//     ring is reused), rounded to bf16 RNE and stored.
+// What limits it (measured, B200): the register file has two banks (even / odd register numbers) and each delivers
+// one new register per cycle; an operand held over from the previous instruction (.reuse) is free.  A scalar FMA
+// with three distinct operands therefore issues every 2 cycles unless one operand is reused, and ptxas interleaves
+// the FMA stream so that about half of them miss (1.5 cycles per FMA; forcing the order through data or control
+// dependencies cost as much in bubbles).  For m <= 4 the kernel stays HBM-bound (21.7 us at m = 1, 22.8 us at m = 4 on
+// the config-3 shape = 96 % / 91 % of the measured HBM peak); at m = 5..8 it is FMA-issue bound (39 us NK, 29 us KN),
+// so TRI_W_NK with 5..8 rows and k <= 4096 goes to the packed-FFMA2 kernel of decode_gemv_m8.cu (24.8 us), whose
+// 64-bit operands read one register of each bank and cannot conflict.
 //
-// TRI_W_KN kernel (W_phys[k][n], N contiguous; secondary path): thread owns 4 adjacent columns and
-// reads them with one coalesced 8-byte load per k; the 16 warps of a CTA split K; same reduction.
+// One kernel, both layouts.  A CTA owns 64 output columns; 4 compute warps + 1 producer warp (160
+// threads), TWO CTAs per SM (18944 = 296 * 64: one wave on 148 SMs), so the prologue, the reduction
+// and the tail of one CTA are covered by its neighbour and, with programmatic dependent launch, by the
+// first CTAs of the next call.
+//   * producer warp (one lane): per 64-k stage one TMA box of W (64 x 64 bf16 = 8 KiB, 128-byte
+//     swizzle, L2 evict-first) and one of X (64 k x 8 rows = 1 KiB; rows >= m and k >= K arrive as
+//     zeros) into a ring of 9 KiB slots; full / empty mbarriers.  X rides in the ring, so there is no
+//     prologue, no limit on K, and nothing but the ring in shared memory.
+//   * compute warps, TRI_W_NK (slot row = column n, 128 B = 64 k): half-warp h of warp w owns the
+//     8-k chunk 2w + h of the stage, lane i of it the columns i, i+16, i+32, i+48: four LDS.128 of
+//     W (the swizzle puts the 8 lanes of a quarter-warp on 8 different 16-byte bank groups), eight
+//     broadcast LDS.128 of X (row mm, same chunk), 4 x 8 x 8 = 256 FMAs.
+//   * compute warps, TRI_W_KN (slot row = k, 128 B = 64 columns n): lane (c = lane & 7, q = lane >> 3)
+//     of warp w owns the 8 columns of chunk c and the k-rows 16w + 4q .. + 3: four LDS.128 of W (a
+//     quarter-warp reads one whole row), eight broadcast LDS.64 of X, 8 x 4 x 8 = 256 FMAs.
+//   * the W registers of stage s + 1 are loaded before the FMAs of stage s, and a slot is released as
+//     soon as its words are in registers.
+//   * after the last stage the partial sums (8 sets for NK, 16 for KN) are added through shared
+//     memory (the ring is dead by then), rounded to bf16 RNE and stored.
 #include "tri_internal.h"
 #include "ptx.cuh"
 
 #include <cuda_bf16.h>
+#include <cstdlib>
 
 namespace tri {
 
-constexpr int GV_M = 8;                 // batch rows per launch (padded with zeros)
-constexpr int GV_COLS = 128;            // output columns per CTA
-constexpr int GV_CWARPS = 12;           // compute warps (3 groups of 4)
-constexpr int GV_GROUPS = 3;
+constexpr int GV_M = 8;                  // batch rows per launch (the X box is always 8 rows; missing rows are zeros)
+constexpr int GV_COLS = 64;              // output columns per CTA
+constexpr int GV_CWARPS = 4;             // compute warps
 constexpr int GV_CTHREADS = GV_CWARPS * 32;
-constexpr int GV_THREADS = (GV_CWARPS + 1) * 32;     // + producer warp
-constexpr int GV_STAGE_K = 64;          // k-values per stage (one TMA box)
-constexpr int GV_SLOT_BYTES = GV_STAGE_K * GV_COLS * 2;   // 16 KiB
-constexpr int GV_MAX_SLOTS = 6;
-constexpr int GV_XCHUNK = 72;           // floats per 8-k chunk of xs (64 used + 8 padding)
-constexpr int GV_SETS = GV_CWARPS * 2;  // half-warp partial sums
-constexpr int GV_SET_STRIDE = GV_M * GV_COLS + 16;   // floats; +16 keeps the two half-warps on different banks
-constexpr int GV_BAR_BYTES = 128;
-constexpr int GV_KMAX = 4096;
+constexpr int GV_THREADS = GV_CTHREADS + 32;          // + producer warp
+constexpr int GV_STAGE_K = 64;           // k-values per stage
+constexpr int GV_W_BYTES = GV_STAGE_K * GV_COLS * 2;  // 8 KiB
+constexpr int GV_X_BYTES = GV_STAGE_K * GV_M * 2;     // 1 KiB
+constexpr int GV_SLOT_BYTES = GV_W_BYTES + GV_X_BYTES;
+constexpr int GV_MAX_SLOTS = 12;
+constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS;
+constexpr int GV_RED_STRIDE = GV_M * GV_COLS + 16;    // floats per partial-sum set; +16 keeps the two half-warps on different banks
 
-__device__ __forceinline__ float2 unpack_bf16x2(uint32_t w)
+__host__ __device__ constexpr size_t gemv_smem_bytes(int nslots)
 {
-    return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
+    return 1024 + (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES;
 }
 
-// Shared memory (from the 1024-aligned base): ring[nslots][16 KiB] | full[6], empty[6] | xs[nchunks][72] floats.
-__host__ __device__ inline size_t gemv_smem_bytes(int nslots, int nstages)
+// acc + w.half * x.half: the sm_100 mixed-precision FMA (SASS FHFMA.BF16; the half selects become operand modifiers of
+// the 32-bit registers, so no unpack instruction is issued).  WH / XH pick the low (0) or high (1) bf16 of the words.
+#define TRI_FMA_BF16(WSEL, XSEL)                                                                                      \
+    asm("{\n\t.reg .b16 wl, wh, xl, xh;\n\tmov.b32 {wl, wh}, %1;\n\tmov.b32 {xl, xh}, %2;\n\t"                      \
+        "fma.rn.f32.bf16 %0, " WSEL ", " XSEL ", %3;\n\t}" : "=f"(d) : "r"(w), "r"(x), "f"(acc))
+template <int WH, int XH>
+__device__ __forceinline__ float fma_bf16(uint32_t w, uint32_t x, float acc)
 {
-    size_t main_bytes = (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES + (size_t)nstages * 8 * GV_XCHUNK * 4;
-    size_t red_bytes = (size_t)GV_SETS * GV_SET_STRIDE * 4;
-    return 1024 + (main_bytes > red_bytes ? main_bytes : red_bytes);
+    float d;
+    if constexpr (WH == 0 && XH == 0) TRI_FMA_BF16("wl", "xl");
+    else if constexpr (WH == 1 && XH == 1) TRI_FMA_BF16("wh", "xh");
+    else if constexpr (WH == 0 && XH == 1) TRI_FMA_BF16("wl", "xh");
+    else TRI_FMA_BF16("wh", "xl");
+    return d;
+}
+#undef TRI_FMA_BF16
+__device__ __forceinline__ void lds128(uint32_t (&r)[4], uint32_t addr)
+{
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+__device__ __forceinline__ void lds64(uint32_t (&r)[2], uint32_t addr)
+{
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(addr));
 }
 
-__global__ void __launch_bounds__(GV_THREADS, 1)
-gemv_nk_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restrict__ x, int64_t ldx,
-               uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k, int nslots)
+// MR: batch rows computed (1, 2, 4 or 8 >= m).  KN: W_phys[k][n] (slot row = k) instead of W_phys[n][k] (slot row = n).
+template <int MR, bool KN>
+__global__ void __launch_bounds__(GV_THREADS, 2)
+gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap xmap, uint16_t *__restrict__ y,
+            int64_t ldy, int m, int n, int k, int nslots)
 {
     extern __shared__ uint8_t smem_raw[];
-    // keep the shared state space visible to the compiler: offset arithmetic on the shared window address
-    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    uint8_t *smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;     // 128-byte swizzle atoms are 1 KiB
+    float *red = reinterpret_cast<float *>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)));
     const uint32_t ring = smem_base;
     const uint32_t full0 = smem_base + nslots * GV_SLOT_BYTES;
     const uint32_t empty0 = full0 + 8 * GV_MAX_SLOTS;
-    const uint32_t xs_addr = full0 + GV_BAR_BYTES;
-    float *xs = reinterpret_cast<float *>(smem + nslots * GV_SLOT_BYTES + GV_BAR_BYTES);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * GV_COLS;
     const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
 
-    // Programmatic dependent launch: let the next kernel of the stream start on SMs as they drain.  The
-    // weight stream (model state, never an output of the preceding kernel) is prefetched at once; X and
-    // Y are touched only after pdl_wait(), i.e. after the preceding grid has completed.
+    // Programmatic dependent launch: the next kernel of the stream may start its CTAs as SM resources free up.
+    // W (model state, never an output of the preceding kernel) is fetched at once; X is fetched and Y is written
+    // only after pdl_wait(), i.e. after the preceding grid has completed (aliasing rule in include/triroof.h).
     ptx::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < nslots; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);
-            ptx::mbar_init(empty0 + 8 * s, 4);       // the 4 warps of the group that consumed the slot
+            ptx::mbar_init(empty0 + 8 * s, GV_CWARPS);
         }
         ptx::fence_mbar_init();
     }
     __syncthreads();
 
     if (warp == GV_CWARPS) {
-        // ===== producer warp: one lane streams the weight panel =====
+        // ===== producer warp: one lane streams the CTA's weight panel and the matching X slices =====
         if (lane == 0) {
             ptx::prefetch_tmap(&wmap);
-            const uint64_t pol = ptx::policy_evict_first();          // weights are read once
-            int slot = 0;
-            uint32_t par = 1;                                        // parity of the slot's previous release
-            for (int s = 0; s < nstages; ++s) {
-                if (s >= nslots) ptx::mbar_wait(empty0 + 8 * slot, par);
-                const uint32_t fb = full0 + 8 * slot;
+            ptx::prefetch_tmap(&xmap);
+            const uint64_t pol_w = ptx::policy_evict_first();          // weights are read once
+            const uint64_t pol_x = ptx::policy_evict_last();           // X is re-read by every CTA
+            const int npre = nstages < nslots ? nstages : nslots;
+            for (int s = 0; s < npre; ++s) {
+                const uint32_t fb = full0 + 8 * s;
                 ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
-                ptx::tma_load_2d_hint(ring + slot * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol);
+                if (KN) ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES, &wmap, n0, s * GV_STAGE_K, fb, pol_w);
+                else ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol_w);
+            }
+            ptx::pdl_wait();
+            for (int s = 0; s < npre; ++s)
+                ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, full0 + 8 * s, pol_x);
+            int slot = 0;
+            uint32_t par = 0;                                          // parity of the slot's first release
+            for (int s = npre; s < nstages; ++s) {
+                ptx::mbar_wait(empty0 + 8 * slot, par);
+                const uint32_t fb = full0 + 8 * slot, dst = ring + slot * GV_SLOT_BYTES;
+                ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
+                if (KN) ptx::tma_load_2d_hint(dst, &wmap, n0, s * GV_STAGE_K, fb, pol_w);
+                else ptx::tma_load_2d_hint(dst, &wmap, s * GV_STAGE_K, n0, fb, pol_w);
+                ptx::tma_load_2d_hint(dst + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, fb, pol_x);
                 if (++slot == nslots) { slot = 0; par ^= 1; }
             }
         }
+        return;
+    }
+
+    // ===== compute warps =====
+    constexpr int NCOL = KN ? 8 : 4;                                  // columns per lane
+    float acc[NCOL][MR];
+#pragma unroll
+    for (int j = 0; j < NCOL; ++j)
+#pragma unroll
+        for (int mm = 0; mm < MR; ++mm) acc[j][mm] = 0.f;
+
+    // NK: half-warp -> 8-k chunk, lane i -> columns i + 16 j.   KN: lane -> (chunk c of 8 columns, k-rows 16 w + 4 q + t).
+    const int i16 = lane & 15, chunk = 2 * warp + (lane >> 4);
+    const int c8 = lane & 7, q4 = lane >> 3, krow = 16 * warp + 4 * q4;
+    uint32_t woff[4], xoff;
+    if (KN) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t) woff[t] = (uint32_t)(krow + t) * 128u + (uint32_t)((c8 ^ ((krow + t) & 7)) << 4);
+        xoff = GV_W_BYTES + (uint32_t)krow * 2u;
     } else {
-        // ===== compute warps =====
-        // X -> fp32 in shared memory: xs[chunk * 72 + kk * 8 + mm]; zero beyond m and beyond k.
-        ptx::pdl_wait();
-        // A thread takes one 8-k chunk of FOUR batch rows: 4 x 16-byte loads (all issued before the first store:
-        // they are L2 hits of ~1 us latency), then 8 x 16-byte stores {x[m0..m0+3][kk]} — conflict free because
-        // consecutive chunks are 72 floats apart.
-        {
-            const int mh = threadIdx.x & 1, nchunks = nstages * 8;
-            constexpr int CSTEP = GV_CTHREADS / 2, XB = 3;            // 192 chunks per pass
-            for (int cb = threadIdx.x >> 1; cb < nchunks; cb += CSTEP * XB) {
-                uint4 v[XB][4];
 #pragma unroll
-                for (int u = 0; u < XB; ++u)
+        for (int j = 0; j < 4; ++j) woff[j] = (uint32_t)(i16 + 16 * j) * 128u + (uint32_t)((chunk ^ (i16 & 7)) << 4);
+        xoff = GV_W_BYTES + (uint32_t)chunk * 16u;
+    }
+
+    uint32_t wv[2][4][4];
+    int slot = 0;
+    uint32_t par = 0;
+    ptx::mbar_wait(full0, 0);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        const int c = cb + u * CSTEP, mm = mh * 4 + r;
-                        v[u][r] = make_uint4(0u, 0u, 0u, 0u);
-                        if (mm < m && 8 * c < k) v[u][r] = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
-                    }
+    for (int j = 0; j < 4; ++j) lds128(wv[0][j], ring + woff[j]);
+
+    auto stage = [&](auto cur_tag, int s) {
+        constexpr int CUR = decltype(cur_tag)::value, NXT = CUR ^ 1;
+        const uint32_t base = ring + slot * GV_SLOT_BYTES;
+        uint32_t xv[MR][KN ? 2 : 4];
 #pragma unroll
-                for (int u = 0; u < XB; ++u) {
-                    const int c = cb + u * CSTEP;
-                    if (c < nchunks) {
-                        float4 *dst = reinterpret_cast<float4 *>(xs + (size_t)c * GV_XCHUNK + mh * 4);
-                        const uint32_t *w0 = &v[u][0].x, *w1 = &v[u][1].x, *w2 = &v[u][2].x, *w3 = &v[u][3].x;
+        for (int mm = 0; mm < MR; ++mm) {
+            if constexpr (KN) lds64(xv[mm], base + xoff + mm * 128);
+            else lds128(xv[mm], base + xoff + mm * 128);
+        }
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);          // this stage's words are in registers: free the slot
+        if (++slot == nslots) { slot = 0; par ^= 1; }
+        if (s + 1 < nstages) {
+            ptx::mbar_wait(full0 + 8 * slot, par);
+            const uint32_t nb = ring + slot * GV_SLOT_BYTES;
 #pragma unroll
-                        for (int pp = 0; pp < 4; ++pp) {              // bf16 pair pp = k-values 2pp, 2pp+1
-                            const float2 a = unpack_bf16x2(w0[pp]), b = unpack_bf16x2(w1[pp]), cc = unpack_bf16x2(w2[pp]),
-                                         d = unpack_bf16x2(w3[pp]);
-                            dst[(2 * pp) * 2] = make_float4(a.x, b.x, cc.x, d.x);        // 8 floats (2 float4) per k
-                            dst[(2 * pp + 1) * 2] = make_float4(a.y, b.y, cc.y, d.y);
+            for (int j = 0; j < 4; ++j) lds128(wv[NXT][j], nb + woff[j]);
+        }
+        if constexpr (KN) {
+#pragma unroll
+            for (int t = 0; t < 4; ++t)                               // k-row of the lane: x word t >> 1, half t & 1
+#pragma unroll
+                for (int u = 0; u < 4; ++u)                           // word u = columns 2u, 2u + 1 of the chunk
+#pragma unroll
+                    for (int mm = 0; mm < MR; ++mm) {
+                        if (t & 1) {
+                            acc[2 * u][mm] = fma_bf16<0, 1>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u][mm]);
+                            acc[2 * u + 1][mm] = fma_bf16<1, 1>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u + 1][mm]);
+                        } else {
+                            acc[2 * u][mm] = fma_bf16<0, 0>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u][mm]);
+                            acc[2 * u + 1][mm] = fma_bf16<1, 0>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u + 1][mm]);
                         }
                     }
-                }
-            }
+        } else {
+#pragma unroll
+            for (int p = 0; p < 4; ++p)                               // word p = k-values 2p, 2p + 1 of the chunk
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int mm = 0; mm < MR; ++mm) {
+                        acc[j][mm] = fma_bf16<0, 0>(wv[CUR][j][p], xv[mm][p], acc[j][mm]);
+                        acc[j][mm] = fma_bf16<1, 1>(wv[CUR][j][p], xv[mm][p], acc[j][mm]);
+                    }
         }
-        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+    };
+    for (int s = 0; s < nstages; s += 2) {
+        stage(std::integral_constant<int, 0>{}, s);
+        if (s + 1 < nstages) stage(std::integral_constant<int, 1>{}, s + 1);
+    }
 
-        float2 acc[8][4];                                             // [column j][batch-row pair q]
+    // ===== add the partial sums through shared memory (every TMA write has landed and been read: the ring is dead) =====
+    constexpr int NSETS = KN ? 16 : 8;
+    asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+    if constexpr (KN) {
+        float *mine = red + (size_t)(warp * 4 + q4) * GV_RED_STRIDE + 8 * c8;
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
-#pragma unroll
-            for (int q = 0; q < 4; ++q) acc[j][q] = make_float2(0.f, 0.f);
-
-        const int group = warp >> 2;
-        const int half = lane >> 4, i = lane & 15;
-        const int chunk = 2 * (warp & 3) + half;                      // 16-byte chunk of the 128-byte weight row
-        const uint32_t woff = (uint32_t)i * 128u + (uint32_t)((chunk ^ (i & 7)) << 4);
-
-        int slot = group % nslots;
-        uint32_t par = (uint32_t)(group / nslots) & 1;
-        for (int s = group; s < nstages; s += GV_GROUPS) {
-            ptx::mbar_wait(full0 + 8 * slot, par);
-            const uint32_t base = ring + slot * GV_SLOT_BYTES + woff;
-            uint4 wv[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j)                               // column i + 16 j is 2048 bytes further
-                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                             : "=r"(wv[j].x), "=r"(wv[j].y), "=r"(wv[j].z), "=r"(wv[j].w)
-                             : "r"(base + j * 2048));
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);      // weights are in registers: free the slot
-
-            const uint32_t xa = xs_addr + (uint32_t)(s * 8 + chunk) * (GV_XCHUNK * 4);
-#pragma unroll
-            for (int p = 0; p < 4; ++p) {                              // k-pairs of the chunk
-                float4 xv[4];                                          // x[2p][0..7], x[2p+1][0..7]
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
-                                 : "=f"(xv[q].x), "=f"(xv[q].y), "=f"(xv[q].z), "=f"(xv[q].w)
-                                 : "r"(xa + p * 64 + q * 16));
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const uint32_t word = p == 0 ? wv[j].x : p == 1 ? wv[j].y : p == 2 ? wv[j].z : wv[j].w;
-                    // PRMT / LOP3 (ALU pipe): a shift would be turned into an IMAD on the FMA pipe, which is the busy one
-                    const float w0 = __uint_as_float(__byte_perm(word, 0u, 0x1044)), w1 = __uint_as_float(word & 0xffff0000u);
-                    const float2 w0b = make_float2(w0, w0), w1b = make_float2(w1, w1);
-                    acc[j][0] = __ffma2_rn(w0b, make_float2(xv[0].x, xv[0].y), acc[j][0]);
-                    acc[j][1] = __ffma2_rn(w0b, make_float2(xv[0].z, xv[0].w), acc[j][1]);
-                    acc[j][2] = __ffma2_rn(w0b, make_float2(xv[1].x, xv[1].y), acc[j][2]);
-                    acc[j][3] = __ffma2_rn(w0b, make_float2(xv[1].z, xv[1].w), acc[j][3]);
-                    acc[j][0] = __ffma2_rn(w1b, make_float2(xv[2].x, xv[2].y), acc[j][0]);
-                    acc[j][1] = __ffma2_rn(w1b, make_float2(xv[2].z, xv[2].w), acc[j][1]);
-                    acc[j][2] = __ffma2_rn(w1b, make_float2(xv[3].x, xv[3].y), acc[j][2]);
-                    acc[j][3] = __ffma2_rn(w1b, make_float2(xv[3].z, xv[3].w), acc[j][3]);
-                }
-            }
-#pragma unroll
-            for (int t = 0; t < GV_GROUPS; ++t)                        // advance GV_GROUPS stages round the ring
-                if (++slot == nslots) { slot = 0; par ^= 1; }
+        for (int mm = 0; mm < MR; ++mm) {
+            *reinterpret_cast<float4 *>(mine + mm * GV_COLS) = make_float4(acc[0][mm], acc[1][mm], acc[2][mm], acc[3][mm]);
+            *reinterpret_cast<float4 *>(mine + mm * GV_COLS + 4) = make_float4(acc[4][mm], acc[5][mm], acc[6][mm], acc[7][mm]);
         }
-
-        // ===== cross-warp reduction through shared memory (ring, barriers and xs are dead now) =====
-        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-        // red[set][(j * 4 + q) * 32 + i * 2 + e] holds the partial sum of column i + 16 j, batch row 2 q + e.
-        float2 *red = reinterpret_cast<float2 *>(smem);
-        float2 *mine = red + (size_t)(warp * 2 + half) * (GV_SET_STRIDE / 2) + i;
+    } else {
+        float *mine = red + (size_t)(warp * 2 + (lane >> 4)) * GV_RED_STRIDE + i16;
 #pragma unroll
-        for (int j = 0; j < 8; ++j)
+        for (int j = 0; j < 4; ++j)
 #pragma unroll
-            for (int q = 0; q < 4; ++q) mine[(j * 4 + q) * 16] = acc[j][q];
-        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-        for (int o = threadIdx.x; o < GV_M * GV_COLS / 2; o += GV_CTHREADS) {
-            float2 sum = make_float2(0.f, 0.f);
+            for (int mm = 0; mm < MR; ++mm) mine[mm * GV_COLS + 16 * j] = acc[j][mm];
+    }
+    asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
+    const int mm = threadIdx.x >> 4, col = (threadIdx.x & 15) * 4;    // 128 threads x 4 outputs = 8 rows x 64 columns
+    if (mm < m && mm < MR && n0 + col < n) {
+        float4 sum = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-            for (int t = 0; t < GV_SETS; ++t) {
-                const float2 v = red[t * (GV_SET_STRIDE / 2) + o];
-                sum.x += v.x;
-                sum.y += v.y;
-            }
-            const int ii = o & 15, q = (o >> 4) & 3, j = o >> 6, col = n0 + ii + 16 * j;
-            if (col < n) {
-                if (2 * q < m) y[(int64_t)(2 * q) * ldy + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum.x));
-                if (2 * q + 1 < m) y[(int64_t)(2 * q + 1) * ldy + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum.y));
-            }
+        for (int t = 0; t < NSETS; ++t) {
+            const float4 v = *reinterpret_cast<const float4 *>(red + (size_t)t * GV_RED_STRIDE + mm * GV_COLS + col);
+            sum.x += v.x; sum.y += v.y; sum.z += v.z; sum.w += v.w;
+        }
+        uint16_t *dst = y + (int64_t)mm * ldy + n0 + col;
+        const uint32_t lo = ptx::pack_bf16x2(sum.x, sum.y), hi = ptx::pack_bf16x2(sum.z, sum.w);
+        if (n0 + col + 4 <= n && (reinterpret_cast<uintptr_t>(dst) & 7) == 0) {
+            *reinterpret_cast<uint2 *>(dst) = make_uint2(lo, hi);
+        } else {
+            const uint16_t e[4] = {(uint16_t)lo, (uint16_t)(lo >> 16), (uint16_t)hi, (uint16_t)(hi >> 16)};
+            for (int c = 0; c < 4 && n0 + col + c < n; ++c) dst[c] = e[c];
         }
     }
 }
 
-// ---- TRI_W_KN: W_phys[k][n] ------------------------------------------------------------------------
-constexpr int KN_WARPS = 16;
-constexpr int KN_THREADS = KN_WARPS * 32;
-constexpr int KN_UNROLL = 8;
-
-__global__ void __launch_bounds__(KN_THREADS, 1)
-gemv_kn_kernel(const uint16_t *__restrict__ w, int64_t ldw, const uint16_t *__restrict__ x, int64_t ldx,
-               uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k)
+template <int MR, bool KN>
+static cudaError_t launch_gemv(const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int m, int n, int k,
+                               int nslots, size_t smem, int blocks, cudaStream_t s)
 {
-    extern __shared__ uint8_t smem_raw[];
-    float *xs = reinterpret_cast<float *>(smem_raw);                  // xs[k][GV_M]
-    float *red = xs + (size_t)k * GV_M;                               // red[warp][mm][col]
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * GV_COLS;
-    const int c0 = n0 + lane * 4;                                     // this thread's 4 columns
-
-    for (int i = threadIdx.x; i < k * GV_M; i += KN_THREADS) {
-        const int mm = i / k, kk = i - mm * k;
-        float v = 0.f;
-        if (mm < m) v = __uint_as_float((uint32_t)x[(int64_t)mm * ldx + kk] << 16);
-        xs[kk * GV_M + mm] = v;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gemv_kernel<MR, KN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
     }
-    __syncthreads();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(blocks);
+    cfg.blockDim = dim3(GV_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, gemv_kernel<MR, KN>, wmap, xmap, y, ldy, m, n, k, nslots);
+}
 
-    float acc[4][GV_M];
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int mm = 0; mm < GV_M; ++mm) acc[j][mm] = 0.f;
-
-    const bool full_cols = (c0 + 3 < n);
-    for (int kb = warp * KN_UNROLL; kb < k; kb += KN_WARPS * KN_UNROLL) {
-        uint2 wv[KN_UNROLL];
-#pragma unroll
-        for (int u = 0; u < KN_UNROLL; ++u) {
-            const int kk = kb + u;
-            wv[u] = make_uint2(0u, 0u);
-            if (kk < k) {
-                const uint16_t *row = w + (int64_t)kk * ldw;
-                if (full_cols) {
-                    wv[u] = __ldcs(reinterpret_cast<const uint2 *>(row + c0));
-                } else {
-                    uint32_t e[4] = {0, 0, 0, 0};
-                    for (int j = 0; j < 4; ++j)
-                        if (c0 + j < n) e[j] = row[c0 + j];
-                    wv[u] = make_uint2(e[0] | (e[1] << 16), e[2] | (e[3] << 16));
-                }
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < KN_UNROLL; ++u) {
-            const int kk = kb + u;
-            if (kk < k) {
-                const float4 xa = *reinterpret_cast<const float4 *>(xs + kk * GV_M);
-                const float4 xb = *reinterpret_cast<const float4 *>(xs + kk * GV_M + 4);
-                const float xv[GV_M] = {xa.x, xa.y, xa.z, xa.w, xb.x, xb.y, xb.z, xb.w};
-                const float2 w01 = unpack_bf16x2(wv[u].x), w23 = unpack_bf16x2(wv[u].y);
-                const float wf[4] = {w01.x, w01.y, w23.x, w23.y};
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-#pragma unroll
-                    for (int mm = 0; mm < GV_M; ++mm) acc[j][mm] = __fmaf_rn(wf[j], xv[mm], acc[j][mm]);
-            }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int mm = 0; mm < GV_M; ++mm) red[(warp * GV_M + mm) * GV_COLS + lane * 4 + j] = acc[j][mm];
-    __syncthreads();
-    for (int o = threadIdx.x; o < GV_M * GV_COLS; o += KN_THREADS) {
-        const int mm = o / GV_COLS, col = o - mm * GV_COLS;
-        float sum = 0.f;
-#pragma unroll
-        for (int wq = 0; wq < KN_WARPS; ++wq) sum += red[(wq * GV_M + mm) * GV_COLS + col];
-        if (mm < m && n0 + col < n) y[(int64_t)mm * ldy + n0 + col] = __bfloat16_as_ushort(__float2bfloat16_rn(sum));
-    }
+template <bool KN>
+static cudaError_t launch_gemv_rows(int mr, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
+                                    int nslots, size_t smem, int blocks, cudaStream_t s)
+{
+    if (mr <= 1) return launch_gemv<1, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
+    if (mr <= 2) return launch_gemv<2, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
+    if (mr <= 4) return launch_gemv<4, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
+    return launch_gemv<8, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
 }
 
 static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
@@ -314,7 +307,6 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
     if (n < 1 || k < 1) return fail(TRI_ERR_INVALID_ARG, "n = %d, k = %d must be positive", n, k);
     if (w_layout != TRI_W_NK && w_layout != TRI_W_KN) return fail(TRI_ERR_INVALID_ARG, "w_layout = %d", w_layout);
     if (k % 8 != 0) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d must be a multiple of 8", k);
-    if (k > GV_KMAX) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d exceeds %d (X must fit shared memory as fp32)", k, GV_KMAX);
     if (ldx < k || ldy < n) return fail(TRI_ERR_INVALID_ARG, "ldx = %lld < k or ldy = %lld < n", (long long)ldx, (long long)ldy);
     if (ldw < (w_layout == TRI_W_NK ? k : n)) return fail(TRI_ERR_INVALID_ARG, "ldw = %lld too small", (long long)ldw);
     if (ldx % 8 != 0 || ldw % 8 != 0) return fail(TRI_ERR_ALIGNMENT, "ldx and ldw must be multiples of 8 elements");
@@ -331,49 +323,45 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
     if (st != TRI_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int blocks = (n + GV_COLS - 1) / GV_COLS;
+    const bool kn = w_layout == TRI_W_KN;
 
-    if (w_layout == TRI_W_NK) {
-        CUtensorMap wmap;
-        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
+    CUtensorMap wmap;
+    if (kn) st = make_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, GV_COLS, GV_STAGE_K, CU_TENSOR_MAP_SWIZZLE_128B);
+    else st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (st != TRI_OK) return st;
+
+    // Ring depth: 8 slots of 9 KiB per CTA = 128 KiB of weights in flight per SM with two CTAs resident (a TMA-only
+    // microbenchmark needed > 48 KiB per SM; 96 KiB and more were equal).  The partial-sum sets reuse the ring, so it
+    // is never smaller than they are.  TRI_GEMV_SLOTS is a debug override.
+    static int slots_cfg = -1;
+    if (slots_cfg < 0) {
+        const char *e = getenv("TRI_GEMV_SLOTS");
+        slots_cfg = e ? atoi(e) : 0;
+        if (slots_cfg < 4 || slots_cfg > GV_MAX_SLOTS) slots_cfg = 8;
+    }
+    const int nslots = slots_cfg;
+    static int force_fhfma = -1;                                     // debug only: TRI_GEMV_FHFMA=1 keeps every shape on this kernel
+    if (force_fhfma < 0) {
+        const char *e = getenv("TRI_GEMV_FHFMA");
+        force_fhfma = e ? atoi(e) : 0;
+    }
+    const size_t smem = gemv_smem_bytes(nslots);
+    static_assert((size_t)4 * GV_SLOT_BYTES >= (size_t)16 * GV_RED_STRIDE * 4, "the partial sums must fit the smallest ring");
+
+    for (int r0 = 0; r0 < m; r0 += GV_M) {
+        const int mr = m - r0 < GV_M ? m - r0 : GV_M;
+        if (!kn && mr > 4 && k <= GEMV_NK8_KMAX && !force_fhfma) {       // FFMA2 kernel: see decode_gemv_m8.cu for why
+            st = launch_gemv_nk8(mr, n, k, x + (int64_t)r0 * ldx, ldx, w, ldw, y + (int64_t)r0 * ldy, ldy, di, s);
+            if (st != TRI_OK) return st;
+            continue;
+        }
+        CUtensorMap xmap;            // X rows r0 .. r0 + mr - 1; the 8-row box is zero-filled beyond them and beyond k
+        st = make_tmap_2d_bf16(&xmap, x + (int64_t)r0 * ldx, (uint64_t)k, (uint64_t)mr, (uint64_t)ldx * 2, GV_STAGE_K, GV_M,
+                               CU_TENSOR_MAP_SWIZZLE_NONE);
         if (st != TRI_OK) return st;
-        const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
-        int nslots = GV_MAX_SLOTS < nstages ? GV_MAX_SLOTS : nstages;       // deepest ring that fits beside xs
-        while (nslots > 2 && gemv_smem_bytes(nslots, nstages) > di->smem_optin) --nslots;
-        const size_t smem = gemv_smem_bytes(nslots, nstages);
-        static bool attr_set = false;
-        if (!attr_set) {
-            TRI_CUDA(cudaFuncSetAttribute(gemv_nk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)di->smem_optin));
-            attr_set = true;
-        }
-        if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
-        for (int r0 = 0; r0 < m; r0 += GV_M) {
-            const int mr = m - r0 < GV_M ? m - r0 : GV_M;
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3(blocks);
-            cfg.blockDim = dim3(GV_THREADS);
-            cfg.dynamicSmemBytes = smem;
-            cfg.stream = s;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-            attr[0].val.programmaticStreamSerializationAllowed = 1;
-            cfg.attrs = attr;
-            cfg.numAttrs = 1;
-            TRI_CUDA(cudaLaunchKernelEx(&cfg, gemv_nk_kernel, wmap, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k,
-                                        nslots));
-        }
-    } else {
-        const size_t smem = ((size_t)k * GV_M + (size_t)KN_WARPS * GV_M * GV_COLS) * 4;
-        static bool attr_set = false;
-        if (!attr_set) {
-            TRI_CUDA(cudaFuncSetAttribute(gemv_kn_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)di->smem_optin));
-            attr_set = true;
-        }
-        if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
-        for (int r0 = 0; r0 < m; r0 += GV_M) {
-            const int mr = m - r0 < GV_M ? m - r0 : GV_M;
-            gemv_kn_kernel<<<blocks, KN_THREADS, smem, s>>>(w, ldw, x + (int64_t)r0 * ldx, ldx, y + (int64_t)r0 * ldy, ldy, mr, n, k);
-            TRI_CUDA(cudaGetLastError());
-        }
+        cudaError_t e = kn ? launch_gemv_rows<true>(mr, wmap, xmap, y + (int64_t)r0 * ldy, ldy, n, k, nslots, smem, blocks, s)
+                           : launch_gemv_rows<false>(mr, wmap, xmap, y + (int64_t)r0 * ldy, ldy, n, k, nslots, smem, blocks, s);
+        if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "decode_gemv launch: %s", cudaGetErrorString(e));
     }
     return TRI_OK;
 }

@@ -28,6 +28,11 @@ int ensure_init(const DeviceInfo **info);
 int make_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer,
                       uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz);
 
+// decode_gemv_m8.cu: the FFMA2 kernel for TRI_W_NK, 5..8 rows, k <= GEMV_NK8_KMAX (x, y offset to the first row).
+constexpr int GEMV_NK8_KMAX = 4096;
+int launch_gemv_nk8(int mr, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, uint16_t *y,
+                    int64_t ldy, const DeviceInfo *di, cudaStream_t s);
+
 inline bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 
 }  // namespace tri

@@ -90,7 +90,7 @@ def test_ones_give_k_exactly(layout, k):
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
 @pytest.mark.parametrize("m,n,k", [(1, 8, 8), (7, 264, 80), (8, 1000, 136), (9, 129, 264), (16, 520, 4096),
-                                   (3, 18944, 128), (8, 127, 3584)])
+                                   (3, 18944, 128), (8, 127, 3584), (2, 72, 18944), (4, 200, 8200), (5, 64, 64), (12, 65, 72)])
 def test_ragged_shapes(layout, m, n, k):
     x = normal_bf16(30 + m, (m, k))
     w = normal_bf16(31 + m, (k, n), 0.05)
