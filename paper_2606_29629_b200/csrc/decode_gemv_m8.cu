@@ -28,7 +28,6 @@ constexpr int GV_XCHUNK = 72;           // floats per 8-k chunk of xs (64 used +
 constexpr int GV_SETS = GV_CWARPS * 2;  // half-warp partial sums
 constexpr int GV_SET_STRIDE = GV_M * GV_COLS + 16;   // floats; +16 keeps the two half-warps on different banks
 constexpr int GV_BAR_BYTES = 128;
-constexpr int GV_KMAX = GEMV_NK8_KMAX;     // X must fit shared memory as fp32
 
 __device__ __forceinline__ float2 unpack_bf16x2(uint32_t w)
 {

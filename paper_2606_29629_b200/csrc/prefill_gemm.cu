@@ -22,6 +22,7 @@
 // W tile is loaded as four 64(n) x 64(k) boxes and described to the MMA with the MN-major descriptor.
 #include "tri_internal.h"
 #include "ptx.cuh"
+#include "gemm_common.cuh"
 
 #include <cstdlib>
 
@@ -35,32 +36,6 @@ constexpr int GM_STAGE_BYTES = GM_A_BYTES + GM_B_BYTES;
 constexpr int GM_THREADS = 256;
 constexpr int GM_TMEM_COLS = 512;
 constexpr int GM_SMEM_BYTES = 1024 + GM_STAGES * GM_STAGE_BYTES + 256;
-
-// Instruction descriptor (PTX ISA, tcgen05.mma kind::f16): D = f32 (bits 4-5 = 1), A = B = bf16
-// (bits 7-9, 10-12 = 1), A K-major (bit 15 = 0), B major in bit 16, N >> 3 in bits 17-22, M >> 4 in 24-28.
-__host__ __device__ constexpr uint32_t make_idesc(int mdim, int ndim, int b_mn_major)
-{
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(ndim >> 3) << 17) |
-           ((uint32_t)(mdim >> 4) << 24);
-}
-
-// Shared-memory matrix descriptor: start address >> 4 (bits 0-13), leading byte offset >> 4 (16-29),
-// stride byte offset >> 4 (32-45), descriptor version 1 (bits 46-47), swizzle mode 2 = 128 B (61-63).
-__device__ __forceinline__ uint64_t make_sdesc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
-{
-    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
-           (1ull << 46) | (2ull << 61);
-}
-
-struct GemmParams {
-    int m, n, k;
-    int tiles_m, tiles_n, kblocks;
-    int64_t ldc;
-    uint16_t *c;
-    int b_mn_major;          // 0: W is [n][k] (K-major);  1: W is [k][n] (MN-major)
-    uint32_t b_lbo, b_sbo;   // descriptor strides of the B operand
-    uint32_t b_kstep;        // byte advance of the B start address per UMMA_K = 16
-};
 
 __global__ void __launch_bounds__(GM_THREADS, 1)
 gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap, const GemmParams p)
@@ -225,18 +200,24 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     int st = ensure_init(&di);
     if (st != TRI_OK) return st;
 
+    // Default: the CTA-pair kernel (prefill_gemm_2sm.cu).  TRI_GEMM_1SM=1 (debug / A-B comparison) keeps the one-CTA kernel.
+    static int one_sm = -1;
+    if (one_sm < 0) { const char *e = getenv("TRI_GEMM_1SM"); one_sm = e ? atoi(e) : 0; }
+    const int bn_box = one_sm ? GM_BN : GM_BN / 2;            // W columns staged per CTA
+    const int rows_per_tile = one_sm ? GM_BM : 2 * GM_BM;
+
     CUtensorMap amap, wmap;
     st = make_tmap_2d_bf16(&amap, a, (uint64_t)k, (uint64_t)m, (uint64_t)lda * 2, GM_BK, GM_BM, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
     GemmParams p;
     p.m = m; p.n = n; p.k = k;
-    p.tiles_m = (m + GM_BM - 1) / GM_BM;
+    p.tiles_m = (m + rows_per_tile - 1) / rows_per_tile;
     p.tiles_n = (n + GM_BN - 1) / GM_BN;
     p.kblocks = (k + GM_BK - 1) / GM_BK;
     p.ldc = ldc;
     p.c = c;
     if (w_layout == TRI_W_NK) {
-        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, GM_BN, CU_TENSOR_MAP_SWIZZLE_128B);
+        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, bn_box, CU_TENSOR_MAP_SWIZZLE_128B);
         p.b_mn_major = 0;
         p.b_lbo = 16; p.b_sbo = 1024; p.b_kstep = 32;     // 8-row groups 1024 B apart; 16 k-values = 32 B
     } else {
@@ -245,11 +226,9 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
         // MN-major, 128-byte swizzle: a 64(n) x 64(k) box is 64 k-rows of 128 B (8 KiB); 8-k groups are
         // 1024 B apart (stride), the next 64 columns of n start 8192 B later (leading); 16 k-values = 2048 B.
         p.b_lbo = 8192; p.b_sbo = 1024; p.b_kstep = 2048;
-        static int swap = -1;                               // debug only: TRI_GEMM_KN_SWAP=1 swaps LBO / SBO
-        if (swap < 0) { const char *e = getenv("TRI_GEMM_KN_SWAP"); swap = e ? atoi(e) : 0; }
-        if (swap) { p.b_lbo = 1024; p.b_sbo = 8192; }
     }
     if (st != TRI_OK) return st;
+    if (!one_sm) return launch_gemm_2sm(amap, wmap, p, di->sm_count, static_cast<cudaStream_t>(stream));
 
     static bool attr_set = false;
     if (!attr_set) {
