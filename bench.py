@@ -32,6 +32,7 @@ KS = [1 << i for i in range(13)]
 GEMV_SHAPE = (8, 18944, 3584)         # m, n, k
 GEMM_SHAPE = (4096, 18944, 3584)
 GEMV_COPIES = 8
+PAPER_KS = [4, 100, 200, 400, 800]      # the paper's own A.I. set {1, 25, 50, 100, 200} FLOP/B
 FP32_LANES_PER_SM = 128                # FP32 FMA lanes per SM (4 SMSPs x 32); DESIGN.md "ALU peak"
 REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
            0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
@@ -210,6 +211,70 @@ def summarise_clocks(samples, peaks):
             "power_w_mean": sum(s["power_w"] for s in busy) / len(busy), "samples": len(busy), "source": "nvml via phase_trace_start"}
 
 
+def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
+    """Per-point sustained pass (outside the timed region): every A.I. point, the paper's own A.I. series and the two
+    phase kernels are looped for `seconds` each while the library's NVML sampler runs; returns, per point, the device
+    time per launch, the SM clock / temperature / power seen during that window and the energy per FLOP and per byte
+    (NVML energy counter read at both ends) — BASELINE.json north_star "SM clock, temperature and joules per op per phase"."""
+    m, n, k = GEMV_SHAPE
+    pm, pn, pk = GEMM_SHAPE
+
+    def gemvs():
+        for w in step.gw:
+            tri.decode_gemv(m, n, k, step.gx, k, w, k, tri.TRI_W_NK, step.gy, n)
+
+    specs = [(f"fma_k{kk}", "sweep", kk, (lambda kk=kk: tri.roofline_run(kk / 4.0, N_FMA, step.x, step.y)), 1, fma_flop(kk), 8.0 * N_FMA)
+             for kk in KS]
+    specs += [(f"paper_ai{kk / 4:g}", "paper_ai", kk, (lambda kk=kk: tri.roofline_run(kk / 4.0, N_FMA, step.x, step.y)), 1,
+               fma_flop(kk), 8.0 * N_FMA) for kk in PAPER_KS]
+    specs.append(("gemv", "phase", None, gemvs, GEMV_COPIES, gemm_flop(GEMV_SHAPE), gemm_bytes(GEMV_SHAPE)))
+    specs.append(("gemm", "phase", None,
+                  lambda: tri.prefill_gemm(pm, pn, pk, step.pa, pk, step.pw, pk, tri.TRI_W_NK, step.pc, pn), 1,
+                  gemm_flop(GEMM_SHAPE), gemm_bytes(GEMM_SHAPE)))
+    try:
+        tracer = tri.PhaseTracer(local, period_us=10000, capacity=1 << 17).start(tri.TRI_PHASE_IDLE)
+    except tri.TriError:
+        return {}
+    out, windows = {}, []
+    for idx, (name, series, kk, fn, per_call, flop, nbytes) in enumerate(specs):
+        est = est_ms.get(name) or (fma_flop(kk) / (0.9 * sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6) * 1e3 + 0.33)
+        batch = max(1, int(20.0 / (est * per_call)))                  # about 20 ms of work per host round trip
+        torch.cuda.synchronize()
+        tracer.mark(100 + idx)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0 = tri.tri_nvml_sample(local)["energy_mj"]
+        t0 = time.perf_counter()
+        a.record()
+        calls = 0
+        while time.perf_counter() - t0 < seconds:
+            for _ in range(batch):
+                fn()
+            calls += batch * per_call
+            torch.cuda.synchronize()
+        b.record()
+        torch.cuda.synchronize()
+        e1 = tri.tri_nvml_sample(local)["energy_mj"]
+        windows.append((name, series, kk, 100 + idx, a.elapsed_time(b), calls, flop, nbytes, (e1 - e0) * 1e-3))
+    samples = tracer.stop()
+    for name, series, kk, tag, ms, calls, flop, nbytes, joule in windows:
+        ss = [x for x in samples if x["phase"] == tag and x["sm_mhz"] > 0]
+        bits = 0
+        for x in ss:
+            bits |= int(x["clk_event_reasons"])
+        per_ms = ms / calls
+        out[name] = {"series": series, "k": kk, "ms_sustained": per_ms, "launches": calls, "window_s": ms * 1e-3,
+                     "gbs_sustained": nbytes / per_ms / 1e6, "tflops_sustained": flop / per_ms / 1e9,
+                     "sm_mhz": statistics.median(x["sm_mhz"] for x in ss) if ss else None,
+                     "mem_mhz": statistics.median(x["mem_mhz"] for x in ss) if ss else None,
+                     "temp_c_max": max(x["temp_c"] for x in ss) if ss else None,
+                     "power_w_mean": sum(x["power_w"] for x in ss) / len(ss) if ss else None,
+                     "reasons": [nm for bit, nm in REASONS.items() if bits & bit and nm != "gpu_idle"],
+                     "j_per_flop": joule / (flop * calls) if joule > 0 else None,
+                     "j_per_byte": joule / (nbytes * calls) if joule > 0 else None,
+                     "j_per_call": joule / calls if joule > 0 else None, "nvml_samples": len(ss)}
+    return out
+
+
 def run_ours(args):
     import torch
     import paper_2606_29629_b200 as tri          # raises if the CUDA library cannot be built / loaded: no fallback
@@ -288,6 +353,41 @@ def run_ours(args):
                    "gbs": gemm_bytes(GEMM_SHAPE) / ms / 1e6, "tflops": gm_tf, "bound": "tensor",
                    "roofline_tflops": peaks["bf16_tflops"], "frac": gm_tf / peaks["bf16_tflops"]})
 
+    # ---- per-point sustained pass: clock, temperature, power, J/op per A.I. point and per phase kernel ----
+    extra_points = []
+    if args.char_seconds > 0 and world == 1:
+        est = {f"fma_k{k}": statistics.median(per[f"fma_k{k}"]) for k in KS}
+        est["gemv"] = statistics.median(per["gemv"]) / GEMV_COPIES
+        est["gemm"] = statistics.median(per["gemm"])
+        ch = characterise(torch, tri, step, local, args.char_seconds, peaks, sms, est)
+
+        def at_clock(pt, c):
+            """Roofline fraction of the sustained rate against the roofline AT THE RECORDED SM CLOCK (BASELINE.json
+            north_star): HBM points are clock-independent, ALU points scale with the clock seen in the window; the
+            tensor point is held against the measured sustained cuBLAS rate (power-capped clock, MEASURED_PEAKS.json)."""
+            if not c:
+                return
+            pt["sustained"] = c
+            alu_at_clock = sms * FP32_LANES_PER_SM * 2 * (c["sm_mhz"] or peaks["sm_max_mhz"]) * 1e6 / 1e12
+            if pt["bound"] == "tensor":
+                roof = peaks["bf16_tflops_sustained"]
+            else:                                                      # CUDA-core kernels: min(A.I. x HBM, FP32 ALUs at the clock seen)
+                roof = min(pt["ai"] * peaks["hbm_gbs"] / 1e3, alu_at_clock)
+            pt["roofline_tflops_at_clock"] = roof
+            pt["frac_sustained_at_clock"] = c["tflops_sustained"] / roof
+
+        for pt in points:
+            key = f"fma_k{pt['k']}" if pt["kernel"] == "fma_chain" else ("gemv" if pt["kernel"] == "decode_gemv" else "gemm")
+            at_clock(pt, ch.get(key))
+        for kk in PAPER_KS:                                            # the paper's x-axis (Fig. 3), labelled extra series
+            c = ch.get(f"paper_ai{kk / 4:g}")
+            if c:
+                hb = kk / 4.0 * peaks["hbm_gbs"] / 1e3
+                pt = {"kernel": "fma_chain", "series": "paper A.I. set {1,25,50,100,200} (PAPER.md line 92)", "k": kk, "ai": kk / 4.0,
+                      "bound": "hbm" if hb < alu_peak else "alu"}
+                at_clock(pt, c)
+                extra_points.append(pt)
+
     # dominant kernel of the step: the FMA-chain kernel at k = 4096 (about half of the step time), ALU-bound
     dom = points[len(KS) - 1]
     traffic = ncu_traffic_bytes("fma_chain", column=len(KS) - 1)
@@ -306,7 +406,7 @@ def run_ours(args):
            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
            "data": "synthetic", "config": workload_config(world), "clocks": dict(clocks, sm_mhz_in_kernel_probe=clk_probe),
-           "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points,
+           "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points, "extra_points": extra_points,
            "min_frac": min(p["frac"] for p in points),
            "energy": {"j_per_step": energy_j / args.steps if energy_j else None,
                       "j_per_flop": energy_j / (STEP_FLOP * args.steps) if energy_j else None,
@@ -377,6 +477,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--char-seconds", type=float, default=0.5,
+                    help="seconds of sustained looping per A.I. point for clock / temperature / J-per-op (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
