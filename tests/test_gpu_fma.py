@@ -35,7 +35,7 @@ def test_config1_bit_exact(k):
 
 
 @pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 7, 1023, 1024, 4096, 4097, 4099, 256 * 16 * 3 + 2, 100003])
-@pytest.mark.parametrize("k", [1, 7, 9, 100])
+@pytest.mark.parametrize("k", [1, 7, 9, 33, 100])
 def test_ragged_sizes_and_odd_k(n, k):
     # tails (n % 4 != 0), partial tiles, k that is neither a power of two nor a multiple of the unroll
     x = uniform_pm1(5, n, stream=3)
