@@ -151,6 +151,21 @@ def workload_config(n_gpus):
 # ----------------------------------------------------------------------------------------------------------
 # GPU arm
 # ----------------------------------------------------------------------------------------------------------
+def max_over_ranks(ms, dist, device):
+    """Device time of the slowest rank (the replicas share nothing, so the job is as slow as its slowest GPU)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(flop_per_step, steps, world, ms):
+    """Aggregate TFLOP/s of `world` independent replicas that each ran `steps` steps in `ms` (max over ranks)."""
+    return flop_per_step * steps * world / (ms * 1e-3) / 1e12
+
+
 class GpuStep:
     """Device buffers (seeded synthetic, generated on the device with the bit-identical integer generator for the
     fp32 stream) and the launch sequence of one step.  Every launch goes through the C ABI binding."""
@@ -322,10 +337,7 @@ def run_ours(args):
     e1 = tri.tri_nvml_sample(local)["energy_mj"] if tracer else 0
     samples = tracer.stop() if tracer else []
     total_ms = t_begin.elapsed_time(t_end)
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, "cuda")
     clk_probe = tri.tri_sm_clock_mhz(2000)
 
     per = {}
@@ -400,7 +412,7 @@ def run_ours(args):
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----
     e2e = run_e2e(torch, tri, step, args, barrier, dist)
 
-    value = STEP_FLOP * args.steps * world / (total_ms * 1e-3) / 1e12
+    value = whole_job_value(STEP_FLOP, args.steps, world, total_ms)
     energy_j = (e1 - e0) * 1e-3 if e1 > e0 else None
     out = {"metric": METRIC, "value": value, "unit": "TFLOP/s (algorithmic, whole step)", "n_gpus": world,
            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
@@ -460,13 +472,9 @@ def run_e2e(torch, tri, step, args, barrier, dist):
     b.record()
     barrier()
     ms = a.elapsed_time(b)
-    world = 1
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        world = dist.get_world_size()
-    return {"value": STEP_FLOP * n * world / (ms * 1e-3) / 1e12, "unit": "TFLOP/s (algorithmic, whole step)",
+    ms = max_over_ranks(ms, dist, "cuda")
+    world = dist.get_world_size() if dist is not None else 1
+    return {"value": whole_job_value(STEP_FLOP, n, world, ms), "unit": "TFLOP/s (algorithmic, whole step)",
             "ms_per_step": ms / n, "steps": n, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
 
 
