@@ -196,6 +196,48 @@ int tri_nvml_sample(int device, tri_sample *out);
  * returns delta(clock64) / delta(globaltimer ns) * 1000 in *mhz.  Blocking (synchronises stream). */
 int tri_sm_clock_mhz(unsigned spin_us, double *mhz, void *stream);
 
+/* ------------------------------------------------------------------------------------------------
+ * f3. A.I.-aware frequency selection (section III-C): the throughput and power
+ *     models the sweep data feed, and the Eq. 6 solver.  HOST functions: no GPU, no NVML; every pointer
+ *     is host memory owned by the caller.  Clocks in MHz, throughput in any one unit (TFLOP/s here),
+ *     A.I. in FLOP/byte, beta in throughput per unit A.I. (bandwidth), eta in throughput per MHz.
+ */
+typedef struct {
+    double eta;             /* peak throughput per MHz: compute roof = eta * f            (Eq. 1)          */
+    double beta;            /* memory coefficient:      memory roof  = beta * ai          (Eq. 1)          */
+    double omega, gamma;    /* saturation term ai / (ai + omega * f^gamma) of Eq. 4; omega = 0 is Eq. 1     */
+    double p_tdp;           /* power cap of Eq. 2 (W)                                                       */
+    int32_t n_f;            /* number of supported clocks                                                   */
+    const double *f_mhz;    /* n_f clocks, strictly ascending (the discrete levels the solver searches)     */
+    const double *p_idle_w; /* P_idle(f) at those clocks                                                    */
+    const double *p_dyn_w;  /* P_dyn(f)  at those clocks                                                    */
+} tri_model;
+
+/* Eq. 4: min(eta f ai / (ai + omega f^gamma), beta ai).  NaN if an argument is not positive / finite. */
+double tri_model_theta(const tri_model *m, double ai, double f_mhz);
+/* Eq. 3: min(eta f / (beta ai), beta ai / (eta f)), in (0, 1]. */
+double tri_model_phi(const tri_model *m, double ai, double f_mhz);
+/* Eq. 2 at the i-th supported clock: min(P_idle[i] + P_dyn[i] * phi(ai, f[i]), P_tdp).  NaN if i is out of range. */
+double tri_model_power(const tri_model *m, double ai, int32_t i);
+/* Eq. 5: duration-weighted A.I. of a phase, sum(d_i ai_i) / sum(d_i); NaN if n == 0 or sum(d) <= 0. */
+double tri_phase_ai(const double *d, const double *ai, size_t n);
+/* Eq. 6: among the supported clocks f <= f_limit_mhz with theta(ai, f) >= (1 - eps) * theta(ai, f_max)
+ * (f_max = the highest supported clock), the one of least modelled power; ties go to the HIGHEST such clock
+ * ("the highest frequency that achieves this lower power").  Solved as the paper does, by binary search over
+ * the discrete levels, which is exact when theta is non-decreasing in f and the modelled power is
+ * non-decreasing in f up to the cap; TRI_ERR_INVALID_ARG if the tables violate that (checked), or
+ * if eps is outside [0, 1), or no clock <= f_limit_mhz exists.  If no clock meets the throughput constraint the
+ * highest clock <= f_limit_mhz is returned (best effort, *feasible = 0).  Outputs: index into f_mhz, and flag. */
+int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double eps, int32_t *index, int32_t *feasible);
+/* Fit of Eq. 4 to n measured points (ai_i, f_i, theta_i) at a caller-chosen gamma: beta = mean of theta / ai over
+ * the points with ai <= ai_mem (memory branch); on the compute branch f / theta = 1 / eta + (omega / eta) * f^gamma / ai
+ * is a straight line, so eta and omega come from the ordinary least-squares line of f / theta against f^gamma / ai over
+ * the points with ai >= ai_cmp (omega is clamped at 0).  Writes m->eta, m->beta, m->omega, m->gamma only.
+ * TRI_ERR_INVALID_ARG if the memory set is empty, the compute set has fewer than 2 distinct abscissae, or a value
+ * is not positive and finite. */
+int tri_fit_theta(const double *ai, const double *f_mhz, const double *theta, size_t n, double ai_mem, double ai_cmp,
+                  double gamma, tri_model *m);
+
 #ifdef __cplusplus
 }
 #endif

@@ -6,8 +6,9 @@ import this package.  It imports nothing from paper_2606_29629_b200 and shares n
 
     fma_chain(x, k, a, b)            SURVEY.md §8(c) Oracle A   (oracle/fma_chain.c)
     gemm_rows(a16, w16, rows, ...)   SURVEY.md §8(c) Oracle B   (oracle/gemm_rows.c)
+    oracle.dvfs_model                row f3: PAPER.md Eq. 1-6 in plain fp64 Python, Eq. 6 by exhaustive search
 
-Parity pins live in tests/test_oracle_fma.py and tests/test_oracle_gemm.py; no function here is
+Parity pins live in tests/test_oracle_fma.py, tests/test_oracle_gemm.py and tests/test_oracle_dvfs.py; no function here is
 "parity unpinned".
 """
 from __future__ import annotations

@@ -1,0 +1,62 @@
+"""ORACLE (test infrastructure) for row f3 — the A.I.-aware frequency selection of PAPER.md section III-C.
+
+Plain fp64 Python, one function per equation, in the paper's notation; the Eq. 6 oracle is BRUTE FORCE over the
+clock list (the product uses the paper's binary search).  Imports nothing from paper_2606_29629_b200.
+
+    theta(ai, f, eta, beta, omega, gamma)      Eq. 4; omega = 0 is Eq. 1 (line 142)
+    phi(ai, f, eta, beta)                      Eq. 3 (line 154)
+    power(ai, f, p_idle, p_dyn, p_tdp, ...)    Eq. 2 (line 148)
+    phase_ai(d, ai)                            Eq. 5 (line 173)
+    solve_clock(...)                           Eq. 6 (line 182), exhaustive
+    fit_theta(...)                             the straight-line fit stated in include/triroof.h, via numpy.polyfit
+
+Pins: tests/test_oracle_dvfs.py (closed forms, limits, the paper's qualitative statements, hand-worked numbers).
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+
+def theta(ai, f, eta, beta, omega=0.0, gamma=0.0):
+    compute = eta * f * (ai / (ai + omega * f ** gamma))
+    memory = beta * ai
+    return min(compute, memory)
+
+
+def phi(ai, f, eta, beta):
+    return min(eta * f / (beta * ai), beta * ai / (eta * f))
+
+
+def power(ai, f, p_idle, p_dyn, p_tdp, eta, beta):
+    return min(p_idle + p_dyn * phi(ai, f, eta, beta), p_tdp)
+
+
+def phase_ai(d, ai):
+    num = sum(di * ai_i for di, ai_i in zip(d, ai))
+    den = sum(d)
+    return num / den if den > 0 else math.nan
+
+
+def solve_clock(ai, f_list, p_idle, p_dyn, p_tdp, eta, beta, omega, gamma, f_limit, eps):
+    """Eq. 6 by exhaustive search: (index, feasible).  Least power among the feasible clocks <= f_limit, ties to the
+    highest clock; no feasible clock -> the highest clock <= f_limit, feasible False."""
+    allowed = [i for i, f in enumerate(f_list) if f <= f_limit]
+    need = (1.0 - eps) * theta(ai, f_list[-1], eta, beta, omega, gamma)
+    feas = [i for i in allowed if theta(ai, f_list[i], eta, beta, omega, gamma) >= need]
+    if not feas:
+        return allowed[-1], False
+    pw = {i: power(ai, f_list[i], p_idle[i], p_dyn[i], p_tdp, eta, beta) for i in feas}
+    pmin = min(pw.values())
+    return max(i for i in feas if pw[i] <= pmin), True
+
+
+def fit_theta(ai, f, th, ai_mem, ai_cmp, gamma):
+    ai, f, th = (np.asarray(v, dtype=np.float64) for v in (ai, f, th))
+    mem, cmp_ = ai <= ai_mem, ai >= ai_cmp
+    beta = float(np.mean(th[mem] / ai[mem]))
+    slope, icpt = np.polyfit(f[cmp_] ** gamma / ai[cmp_], f[cmp_] / th[cmp_], 1)
+    if slope < 0:
+        slope, icpt = 0.0, float(np.mean(f[cmp_] / th[cmp_]))
+    return {"eta": 1.0 / icpt, "beta": beta, "omega": slope / icpt, "gamma": gamma}

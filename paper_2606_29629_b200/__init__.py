@@ -39,13 +39,20 @@ B_DEFAULT = 0.0009765625
 EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "tri_sm_count", "tri_l2_bytes",
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
-           "tri_sm_clock_mhz"]
+           "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_solve_clock",
+           "tri_fit_theta"]
 
 
 class TriError(RuntimeError):
     def __init__(self, status: int, name: str, detail: str):
         self.status = status
         super().__init__(f"{name}: status {status} ({detail})")
+
+
+class tri_model(Structure):
+    """include/triroof.h tri_model (f3: PAPER.md Eq. 1-4 parameters + the P_idle / P_dyn tables on the clock list)."""
+    _fields_ = [("eta", c_double), ("beta", c_double), ("omega", c_double), ("gamma", c_double), ("p_tdp", c_double),
+                ("n_f", c_int32), ("f_mhz", POINTER(c_double)), ("p_idle_w", POINTER(c_double)), ("p_dyn_w", POINTER(c_double))]
 
 
 class tri_sample(Structure):
@@ -108,6 +115,16 @@ def lib():
     L.tri_reset_clocks.argtypes = [c_int]
     L.tri_nvml_sample.argtypes = [c_int, POINTER(tri_sample)]
     L.tri_sm_clock_mhz.argtypes = [c_uint, POINTER(c_double), c_void_p]
+    for name in ("tri_model_theta", "tri_model_phi"):
+        getattr(L, name).argtypes = [POINTER(tri_model), c_double, c_double]
+        getattr(L, name).restype = c_double
+    L.tri_model_power.argtypes = [POINTER(tri_model), c_double, c_int32]
+    L.tri_model_power.restype = c_double
+    L.tri_phase_ai.argtypes = [POINTER(c_double), POINTER(c_double), c_size_t]
+    L.tri_phase_ai.restype = c_double
+    L.tri_solve_clock.argtypes = [POINTER(tri_model), c_double, c_double, c_double, POINTER(c_int32), POINTER(c_int32)]
+    L.tri_fit_theta.argtypes = [POINTER(c_double), POINTER(c_double), POINTER(c_double), c_size_t, c_double, c_double, c_double,
+                                POINTER(tri_model)]
     for name in EXPORTS:
         if getattr(L, name).restype is None and name not in ("tri_shutdown",):
             getattr(L, name).restype = c_int
@@ -266,3 +283,45 @@ def phase_trace(pm, pn, pk, pa, pw, pc, dm, dn, dk, dx, dw_list, dy, w_layout=TR
         d["phase_name"] = PHASE_NAMES.get(q.phase, str(q.phase))
         summaries.append(d)
     return samples, summaries
+
+
+# ---- f3: A.I.-aware frequency selection (host functions; argument marshalling only) ----------------------------
+class Model:
+    """Owns the ctypes arrays behind a tri_model."""
+
+    def __init__(self, eta, beta, omega=0.0, gamma=0.0, p_tdp=1000.0, f_mhz=(), p_idle_w=(), p_dyn_w=()):
+        n = len(f_mhz)
+        self._f = (c_double * n)(*f_mhz)
+        self._pi = (c_double * n)(*p_idle_w)
+        self._pd = (c_double * n)(*p_dyn_w)
+        self.c = tri_model(eta, beta, omega, gamma, p_tdp, n, ctypes.cast(self._f, POINTER(c_double)),
+                           ctypes.cast(self._pi, POINTER(c_double)), ctypes.cast(self._pd, POINTER(c_double)))
+
+    def theta(self, ai, f_mhz):
+        return lib().tri_model_theta(byref(self.c), ai, f_mhz)
+
+    def phi(self, ai, f_mhz):
+        return lib().tri_model_phi(byref(self.c), ai, f_mhz)
+
+    def power(self, ai, i):
+        return lib().tri_model_power(byref(self.c), ai, i)
+
+    def solve_clock(self, ai, f_limit_mhz, eps):
+        """Eq. 6 -> (index into f_mhz, feasible)."""
+        idx, feas = c_int32(-1), c_int32(0)
+        _check(lib().tri_solve_clock(byref(self.c), ai, f_limit_mhz, eps, byref(idx), byref(feas)), "tri_solve_clock")
+        return idx.value, bool(feas.value)
+
+
+def tri_phase_ai(durations, ais) -> float:
+    n = len(durations)
+    return lib().tri_phase_ai((c_double * n)(*durations), (c_double * n)(*ais), n)
+
+
+def tri_fit_theta(ai, f_mhz, theta, ai_mem, ai_cmp, gamma=0.0):
+    """Eq. 4 fit -> dict(eta, beta, omega, gamma)."""
+    n = len(ai)
+    m = tri_model()
+    _check(lib().tri_fit_theta((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*theta), n, ai_mem, ai_cmp, gamma,
+                               byref(m)), "tri_fit_theta")
+    return {"eta": m.eta, "beta": m.beta, "omega": m.omega, "gamma": m.gamma}

@@ -1,0 +1,94 @@
+"""Row f3 through the C ABI (host functions, no GPU): tri_model_* / tri_phase_ai / tri_solve_clock / tri_fit_theta against
+oracle/dvfs_model.py on seeded random models — the binary search of Eq. 6 against the oracle's exhaustive search."""
+import math
+
+import numpy as np
+import pytest
+
+import paper_2606_29629_b200 as tri
+from oracle import dvfs_model as o
+
+
+def random_model(rng, n_f=None):
+    n_f = n_f or int(rng.integers(1, 40))
+    f = np.cumsum(rng.uniform(15.0, 120.0, n_f)) + rng.uniform(200.0, 600.0)
+    eta, beta = rng.uniform(0.01, 0.06), rng.uniform(0.5, 8.0)
+    omega, gamma = (0.0, 0.0) if rng.random() < 0.3 else (rng.uniform(0.0, 0.05), rng.uniform(0.0, 1.0))
+    p_idle = np.sort(rng.uniform(40.0, 150.0, n_f))
+    # P_dyn ~ c f^a with a >= 2 keeps P_idle + P_dyn * phi non-decreasing in f on both branches (phi ~ f or 1 / f)
+    p_dyn = rng.uniform(1e-5, 4e-4) * f ** rng.uniform(2.0, 3.0)
+    p_tdp = rng.choice([1e9, rng.uniform(150.0, 900.0)])
+    return dict(eta=eta, beta=beta, omega=omega, gamma=gamma, p_tdp=float(p_tdp), f_mhz=list(f), p_idle_w=list(p_idle), p_dyn_w=list(p_dyn))
+
+
+def test_model_functions_match_oracle():
+    rng = np.random.default_rng(11)
+    for _ in range(200):
+        kw = random_model(rng)
+        m = tri.Model(**kw)
+        for ai in np.exp(rng.uniform(math.log(0.1), math.log(4000.0), 8)):
+            i = int(rng.integers(0, len(kw["f_mhz"])))
+            f = kw["f_mhz"][i]
+            assert m.theta(ai, f) == pytest.approx(o.theta(ai, f, kw["eta"], kw["beta"], kw["omega"], kw["gamma"]), rel=1e-13)
+            assert m.phi(ai, f) == pytest.approx(o.phi(ai, f, kw["eta"], kw["beta"]), rel=1e-13)
+            assert m.power(ai, i) == pytest.approx(o.power(ai, f, kw["p_idle_w"][i], kw["p_dyn_w"][i], kw["p_tdp"], kw["eta"], kw["beta"]), rel=1e-13)
+    assert math.isnan(m.theta(-1.0, 1000.0)) and math.isnan(m.power(1.0, 10 ** 6))
+
+
+def test_phase_ai_matches_oracle_and_config_values():
+    rng = np.random.default_rng(12)
+    for n in (1, 2, 3, 17, 1000):
+        d, a = rng.uniform(0.0, 5.0, n), rng.uniform(0.1, 2000.0, n)
+        assert tri.tri_phase_ai(list(d), list(a)) == pytest.approx(o.phase_ai(d, a), rel=1e-12)
+    assert math.isnan(tri.tri_phase_ai([0.0, 0.0], [1.0, 2.0]))
+    # the three kernels of this library: 2 s of GEMM (A.I. 1736.3) and 2 s of GEMV (7.98) -> 872.1
+    assert tri.tri_phase_ai([2.0, 2.0], [1736.275, 7.979]) == pytest.approx(872.127)
+
+
+def test_solver_binary_search_equals_exhaustive_search():
+    rng = np.random.default_rng(13)
+    checked = rejected = 0
+    for _ in range(3000):
+        kw = random_model(rng)
+        m = tri.Model(**kw)
+        ai = float(np.exp(rng.uniform(math.log(0.1), math.log(4000.0))))
+        f_limit = float(rng.choice([kw["f_mhz"][-1], rng.uniform(kw["f_mhz"][0], kw["f_mhz"][-1] + 50.0)]))
+        eps = float(rng.choice([0.0, 0.02, 0.05, 0.2, rng.uniform(0.0, 0.9)]))
+        try:
+            got = m.solve_clock(ai, f_limit, eps)
+        except tri.TriError as e:                       # the library refuses tables on which the binary search is not exact
+            assert e.status == tri.TRI_ERR_INVALID_ARG
+            f, th = kw["f_mhz"], [o.theta(ai, x, kw["eta"], kw["beta"], kw["omega"], kw["gamma"]) for x in kw["f_mhz"]]
+            pw = [o.power(ai, x, kw["p_idle_w"][i], kw["p_dyn_w"][i], kw["p_tdp"], kw["eta"], kw["beta"]) for i, x in enumerate(f)]
+            assert any(b < a for a, b in zip(th, th[1:])) or any(b < a for a, b in zip(pw, pw[1:]))
+            rejected += 1
+            continue
+        want = o.solve_clock(ai, kw["f_mhz"], kw["p_idle_w"], kw["p_dyn_w"], kw["p_tdp"], kw["eta"], kw["beta"], kw["omega"],
+                             kw["gamma"], f_limit, eps)
+        assert got == want, (kw, ai, f_limit, eps)
+        checked += 1
+    assert checked > 2000, (checked, rejected)
+
+
+def test_solver_argument_errors():
+    kw = random_model(np.random.default_rng(14), n_f=8)
+    m = tri.Model(**kw)
+    for bad in [(-1.0, 2000.0, 0.05), (1.0, 2000.0, 1.0), (1.0, 2000.0, -0.1), (1.0, kw["f_mhz"][0] - 1.0, 0.05)]:
+        with pytest.raises(tri.TriError):
+            m.solve_clock(*bad)
+    kw["f_mhz"][3] = kw["f_mhz"][2]                     # not strictly ascending
+    with pytest.raises(tri.TriError):
+        tri.Model(**kw).solve_clock(1.0, 5000.0, 0.05)
+
+
+def test_fit_matches_oracle_on_noisy_sweep():
+    rng = np.random.default_rng(15)
+    ai = np.array([0.25 * 2 ** i for i in range(13)])
+    f = rng.uniform(1550.0, 1965.0, ai.size)
+    th = np.array([o.theta(a, x, 0.0379, 6.54, 0.02, 0.5) for a, x in zip(ai, f)]) * rng.uniform(0.97, 1.03, ai.size)
+    got = tri.tri_fit_theta(list(ai), list(f), list(th), ai_mem=4.0, ai_cmp=32.0, gamma=0.5)
+    want = o.fit_theta(ai, f, th, 4.0, 32.0, 0.5)
+    for key in ("eta", "beta", "omega", "gamma"):
+        assert got[key] == pytest.approx(want[key], rel=1e-7, abs=1e-12), key
+    with pytest.raises(tri.TriError):
+        tri.tri_fit_theta([1.0, 2.0], [1000.0, 1000.0], [1.0, 2.0], ai_mem=4.0, ai_cmp=32.0)

@@ -1,0 +1,95 @@
+"""Pins of oracle/dvfs_model.py (row f3) against what PAPER.md section III-C and the mathematics fix — not against
+itself: hand-worked numbers, closed forms, limits and the paper's qualitative statements about Fig. 3."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import dvfs_model as o
+
+ETA, BETA = 0.04, 6.5            # TFLOP/s per MHz, TFLOP/s per (FLOP/B): ridge at ai = eta f / beta
+
+
+def test_eq1_hand_worked_values():
+    # f = 1000 MHz: compute roof 40, ridge at ai = 40 / 6.5.  ai = 2 -> memory bound 13; ai = 10 -> compute bound 40
+    assert o.theta(2.0, 1000.0, ETA, BETA) == pytest.approx(13.0, rel=1e-15)
+    assert o.theta(10.0, 1000.0, ETA, BETA) == pytest.approx(40.0, rel=1e-15)
+    assert o.theta(40.0 / 6.5, 1000.0, ETA, BETA) == pytest.approx(40.0, rel=1e-12)      # the ridge: both branches meet
+
+
+def test_eq4_saturation_term():
+    # omega f^gamma = 0.5 * 1000^0.5 = 15.811...; ai = 50: eta f ai / (ai + 15.81) = 40 * 50 / 65.811 = 30.3899...
+    v = o.theta(50.0, 1000.0, ETA, BETA, omega=0.5, gamma=0.5)
+    assert v == pytest.approx(40.0 * 50.0 / (50.0 + 0.5 * math.sqrt(1000.0)), rel=1e-15)
+    assert v == pytest.approx(30.38988, rel=1e-6)                                          # 2000 / 65.8114
+    # "slowly converges to 1 as A.I. increases to infinity, thus reaching the real roofline"
+    assert o.theta(1e12, 1000.0, ETA, 1e9, omega=0.5, gamma=0.5) == pytest.approx(40.0, rel=1e-9)
+    # omega = 0 reduces Eq. 4 to Eq. 1 exactly
+    for ai in (0.25, 3.0, 6.15, 7.0, 1024.0):
+        assert o.theta(ai, 1337.0, ETA, BETA, 0.0, 3.0) == o.theta(ai, 1337.0, ETA, BETA)
+    # throughput still rises with A.I. in the compute-bound regime and never exceeds either roof
+    a = [o.theta(ai, 1000.0, ETA, BETA, 0.5, 0.5) for ai in (20, 40, 80, 160, 320)]
+    assert all(x < y for x, y in zip(a, a[1:])) and max(a) < 40.0
+
+
+def test_eq3_utilisation_peaks_at_the_ridge():
+    f = 1500.0
+    ridge = ETA * f / BETA
+    assert o.phi(ridge, f, ETA, BETA) == pytest.approx(1.0, rel=1e-12)
+    assert o.phi(ridge / 4, f, ETA, BETA) == pytest.approx(0.25, rel=1e-12)               # memory bound: beta ai / (eta f)
+    assert o.phi(ridge * 4, f, ETA, BETA) == pytest.approx(0.25, rel=1e-12)               # compute bound: eta f / (beta ai)
+    xs = np.geomspace(0.1, 1000, 200)
+    assert all(0 < o.phi(x, f, ETA, BETA) <= 1 for x in xs)
+    # symmetric in log(ai) about the ridge
+    assert o.phi(ridge * 3.7, f, ETA, BETA) == pytest.approx(o.phi(ridge / 3.7, f, ETA, BETA), rel=1e-12)
+
+
+def test_eq2_power_rises_to_the_ridge_then_falls_and_is_capped():
+    f, p_idle, p_dyn = 1500.0, 200.0, 600.0
+    ridge = ETA * f / BETA
+    ais = [ridge / 8, ridge / 2, ridge, ridge * 2, ridge * 8]
+    p = [o.power(a, f, p_idle, p_dyn, 1e9, ETA, BETA) for a in ais]
+    assert p[0] < p[1] < p[2] > p[3] > p[4]                                               # peak where both are stressed
+    assert p[2] == pytest.approx(800.0) and p[0] == pytest.approx(200.0 + 600.0 / 8)
+    assert o.power(ridge, f, p_idle, p_dyn, 700.0, ETA, BETA) == 700.0                    # min(., P_TDP)
+
+
+def test_eq5_duration_weighted_mean():
+    assert o.phase_ai([1.0, 3.0], [8.0, 1736.0]) == pytest.approx((8.0 + 3 * 1736.0) / 4)
+    assert o.phase_ai([2.0, 2.0, 2.0], [1.0, 2.0, 6.0]) == pytest.approx(3.0)            # equal durations: plain mean
+    assert o.phase_ai([5.0], [42.0]) == 42.0
+    assert o.phase_ai([0.0, 7.0], [1e9, 3.0]) == 3.0                                      # zero-duration kernels do not count
+    assert math.isnan(o.phase_ai([0.0], [1.0]))
+
+
+def _tables(n=16):
+    f = [450.0 + 100.0 * i for i in range(n)]
+    p_idle = [60.0 + 0.05 * x for x in f]
+    p_dyn = [2e-4 * x * x for x in f]                                                     # ~ f^2: power rises with the clock
+    return f, p_idle, p_dyn
+
+
+def test_eq6_worked_cases():
+    f, pi, pd = _tables()
+    # memory bound (ai far below every ridge): theta = beta ai at every clock -> the LOWEST clock is feasible and cheapest
+    # (Observation 2b: "that same throughput is achievable with the lowest clock")
+    assert o.solve_clock(0.25, f, pi, pd, 1e9, ETA, BETA, 0, 0, f[-1], 0.05) == (0, True)
+    # compute bound: theta = eta f, need (1 - eps) eta f_max -> lowest clock >= 0.95 * 1950 = 1852.5 -> 1950 only
+    assert o.solve_clock(1e4, f, pi, pd, 1e9, ETA, BETA, 0, 0, f[-1], 0.05) == (len(f) - 1, True)
+    assert o.solve_clock(1e4, f, pi, pd, 1e9, ETA, BETA, 0, 0, f[-1], 0.11) == (13, True)               # 0.89 * 1950 = 1735.5 -> 1750 = f[13]
+    # f_limit below the feasible set: best effort, flagged
+    assert o.solve_clock(1e4, f, pi, pd, 1e9, ETA, BETA, 0, 0, 1000.0, 0.05) == (5, False)              # 950 is the highest <= 1000
+    # a power cap flattens the top: all capped clocks tie, the HIGHEST of the tying feasible clocks wins
+    i, ok = o.solve_clock(1e4, f, pi, pd, 100.0, ETA, BETA, 0, 0, f[-1], 0.5)
+    assert ok and i == len(f) - 1
+
+
+def test_fit_recovers_planted_parameters():
+    rng = np.random.default_rng(7)
+    eta, beta, omega, gamma = 0.0379, 6.54, 0.02, 0.5        # omega f^gamma ~ 0.85 FLOP/B: the low-A.I. points stay memory bound
+    ai = np.array([0.25, 0.5, 1, 2, 64, 128, 256, 512, 1024], float)
+    f = rng.uniform(1500, 1965, ai.size)
+    th = np.array([o.theta(a, x, eta, beta, omega, gamma) for a, x in zip(ai, f)])
+    got = o.fit_theta(ai, f, th, ai_mem=2, ai_cmp=64, gamma=gamma)
+    assert got["eta"] == pytest.approx(eta, rel=1e-6) and got["beta"] == pytest.approx(beta, rel=1e-12)
+    assert got["omega"] == pytest.approx(omega, rel=1e-5)
