@@ -22,11 +22,9 @@ constexpr int GV_GROUPS = 3;
 constexpr int GV_CTHREADS = GV_CWARPS * 32;
 constexpr int GV_THREADS = (GV_CWARPS + 1) * 32;     // + producer warp
 constexpr int GV_STAGE_K = 64;          // k-values per stage (one TMA box)
-constexpr int GV_W_BYTES = GV_STAGE_K * GV_COLS * 2;      // 16 KiB of weights per stage
-constexpr int GV_X_BYTES = GV_STAGE_K * GV_M * 2;         // 1 KiB: the stage's slice of X, bf16 [8 rows][64 k]
-constexpr int GV_SLOT_BYTES = GV_W_BYTES + GV_X_BYTES;
-constexpr int GV_MAX_SLOTS = 8;
-constexpr int GV_XCHUNK = 72;           // floats per half-warp scratch buffer: x[8 k][8 rows] fp32 (64 used + 8 padding against bank conflicts)
+constexpr int GV_SLOT_BYTES = GV_STAGE_K * GV_COLS * 2;   // 16 KiB
+constexpr int GV_MAX_SLOTS = 6;
+constexpr int GV_XCHUNK = 72;           // floats per 8-k chunk of xs (64 used + 8 padding)
 constexpr int GV_SETS = GV_CWARPS * 2;  // half-warp partial sums
 constexpr int GV_SET_STRIDE = GV_M * GV_COLS + 16;   // floats; +16 keeps the two half-warps on different banks
 constexpr int GV_BAR_BYTES = 128;
@@ -36,17 +34,17 @@ __device__ __forceinline__ float2 unpack_bf16x2(uint32_t w)
     return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
 }
 
-// Shared memory (from the 1024-aligned base): ring[nslots][17 KiB] | full[8], empty[8] | scratch[24 half-warps][2][72] floats.
-__host__ __device__ inline size_t gemv_smem_bytes(int nslots)
+// Shared memory (from the 1024-aligned base): ring[nslots][16 KiB] | full[6], empty[6] | xs[nchunks][72] floats.
+__host__ __device__ inline size_t gemv_smem_bytes(int nslots, int nstages)
 {
-    size_t main_bytes = (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES + (size_t)GV_SETS * 2 * GV_XCHUNK * 4;
+    size_t main_bytes = (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES + (size_t)nstages * 8 * GV_XCHUNK * 4;
     size_t red_bytes = (size_t)GV_SETS * GV_SET_STRIDE * 4;
     return 1024 + (main_bytes > red_bytes ? main_bytes : red_bytes);
 }
 
 __global__ void __launch_bounds__(GV_THREADS, 1)
-gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap xmap,
-                uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k, int nslots)
+gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const uint16_t *__restrict__ x, int64_t ldx,
+               uint16_t *__restrict__ y, int64_t ldy, int m, int n, int k, int nslots)
 {
     extern __shared__ uint8_t smem_raw[];
     // keep the shared state space visible to the compiler: offset arithmetic on the shared window address
@@ -55,7 +53,8 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
     const uint32_t ring = smem_base;
     const uint32_t full0 = smem_base + nslots * GV_SLOT_BYTES;
     const uint32_t empty0 = full0 + 8 * GV_MAX_SLOTS;
-    const uint32_t xs_addr = full0 + GV_BAR_BYTES;            // per half-warp fp32 scratch for the stage's X chunk
+    const uint32_t xs_addr = full0 + GV_BAR_BYTES;
+    float *xs = reinterpret_cast<float *>(smem + nslots * GV_SLOT_BYTES + GV_BAR_BYTES);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * GV_COLS;
@@ -75,33 +74,59 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
     __syncthreads();
 
     if (warp == GV_CWARPS) {
-        // ===== producer warp: one lane streams the weight panel and the matching slices of X =====
+        // ===== producer warp: one lane streams the weight panel =====
         if (lane == 0) {
             ptx::prefetch_tmap(&wmap);
-            ptx::prefetch_tmap(&xmap);
-            const uint64_t pol_w = ptx::policy_evict_first();        // weights are read once
-            const uint64_t pol_x = ptx::policy_evict_last();         // X is re-read by every CTA
-            const int npre = nstages < nslots ? nstages : nslots;
-            for (int s = 0; s < npre; ++s) {                         // weights first: they do not depend on the preceding kernel
-                ptx::mbar_arrive_expect_tx(full0 + 8 * s, GV_SLOT_BYTES);
-                ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, full0 + 8 * s, pol_w);
-            }
-            ptx::pdl_wait();
-            for (int s = 0; s < npre; ++s)
-                ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, full0 + 8 * s, pol_x);
+            const uint64_t pol = ptx::policy_evict_first();          // weights are read once
             int slot = 0;
-            uint32_t par = 0;                                        // parity of the slot's first release
-            for (int s = npre; s < nstages; ++s) {
-                ptx::mbar_wait(empty0 + 8 * slot, par);
-                const uint32_t fb = full0 + 8 * slot, dst = ring + slot * GV_SLOT_BYTES;
+            uint32_t par = 1;                                        // parity of the slot's previous release
+            for (int s = 0; s < nstages; ++s) {
+                if (s >= nslots) ptx::mbar_wait(empty0 + 8 * slot, par);
+                const uint32_t fb = full0 + 8 * slot;
                 ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
-                ptx::tma_load_2d_hint(dst, &wmap, s * GV_STAGE_K, n0, fb, pol_w);
-                ptx::tma_load_2d_hint(dst + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, fb, pol_x);
+                ptx::tma_load_2d_hint(ring + slot * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol);
                 if (++slot == nslots) { slot = 0; par ^= 1; }
             }
         }
     } else {
         // ===== compute warps =====
+        // X -> fp32 in shared memory: xs[chunk * 72 + kk * 8 + mm]; zero beyond m and beyond k.
+        ptx::pdl_wait();
+        // A thread takes one 8-k chunk of FOUR batch rows: 4 x 16-byte loads (all issued before the first store:
+        // they are L2 hits of ~1 us latency), then 8 x 16-byte stores {x[m0..m0+3][kk]} — conflict free because
+        // consecutive chunks are 72 floats apart.
+        {
+            const int mh = threadIdx.x & 1, nchunks = nstages * 8;
+            constexpr int CSTEP = GV_CTHREADS / 2, XB = 3;            // 192 chunks per pass
+            for (int cb = threadIdx.x >> 1; cb < nchunks; cb += CSTEP * XB) {
+                uint4 v[XB][4];
+#pragma unroll
+                for (int u = 0; u < XB; ++u)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const int c = cb + u * CSTEP, mm = mh * 4 + r;
+                        v[u][r] = make_uint4(0u, 0u, 0u, 0u);
+                        if (mm < m && 8 * c < k) v[u][r] = __ldg(reinterpret_cast<const uint4 *>(x + (int64_t)mm * ldx + 8 * c));
+                    }
+#pragma unroll
+                for (int u = 0; u < XB; ++u) {
+                    const int c = cb + u * CSTEP;
+                    if (c < nchunks) {
+                        float4 *dst = reinterpret_cast<float4 *>(xs + (size_t)c * GV_XCHUNK + mh * 4);
+                        const uint32_t *w0 = &v[u][0].x, *w1 = &v[u][1].x, *w2 = &v[u][2].x, *w3 = &v[u][3].x;
+#pragma unroll
+                        for (int pp = 0; pp < 4; ++pp) {              // bf16 pair pp = k-values 2pp, 2pp+1
+                            const float2 a = unpack_bf16x2(w0[pp]), b = unpack_bf16x2(w1[pp]), cc = unpack_bf16x2(w2[pp]),
+                                         d = unpack_bf16x2(w3[pp]);
+                            dst[(2 * pp) * 2] = make_float4(a.x, b.x, cc.x, d.x);        // 8 floats (2 float4) per k
+                            dst[(2 * pp + 1) * 2] = make_float4(a.y, b.y, cc.y, d.y);
+                        }
+                    }
+                }
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
+
         float2 acc[8][4];                                             // [column j][batch-row pair q]
 #pragma unroll
         for (int j = 0; j < 8; ++j)
@@ -112,36 +137,12 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
         const int half = lane >> 4, i = lane & 15;
         const int chunk = 2 * (warp & 3) + half;                      // 16-byte chunk of the 128-byte weight row
         const uint32_t woff = (uint32_t)i * 128u + (uint32_t)((chunk ^ (i & 7)) << 4);
-        const int kp = i >> 2, mq = i & 3;                            // conversion role of the lane inside its half-warp
-        const uint32_t xraw_off = GV_W_BYTES + (uint32_t)(2 * mq) * 128u + (uint32_t)chunk * 16u + (uint32_t)kp * 4u;
-        const uint32_t xs_half = xs_addr + (uint32_t)(warp * 2 + half) * (2 * GV_XCHUNK * 4);   // two buffers of 72 floats
-        const uint32_t xs_st = xs_half + (uint32_t)(2 * kp) * 32u + (uint32_t)mq * 8u;   // x[2 kp][2 mq]; x[2 kp + 1][..] is 32 B on
-
-        // The half-warp's X chunk of a stage: rows 2 mq, 2 mq + 1, k-pair kp (bf16 pairs, as TMA left them), widened
-        // to fp32 into scratch buffer `buf` as x[kk][row].  Called for the group's NEXT stage: before the FMAs of the
-        // current one if that stage has already landed (the load -> store -> load chain is then off the critical
-        // path), after them otherwise (never waiting ahead of the FMAs keeps the whole ring depth for HBM latency).
-        auto convert_x = [&](int sl, uint32_t buf) {
-            uint32_t xr0, xr1;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(xr0) : "r"(ring + sl * GV_SLOT_BYTES + xraw_off));
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(xr1) : "r"(ring + sl * GV_SLOT_BYTES + xraw_off + 128));
-            const float2 r0 = unpack_bf16x2(xr0), r1 = unpack_bf16x2(xr1);
-            const uint32_t dst = xs_st + buf * (GV_XCHUNK * 4);
-            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(dst), "f"(r0.x), "f"(r1.x) : "memory");
-            asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(dst + 32), "f"(r0.y), "f"(r1.y) : "memory");
-        };
 
         int slot = group % nslots;
         uint32_t par = (uint32_t)(group / nslots) & 1;
-        if (group < nstages) {
+        for (int s = group; s < nstages; s += GV_GROUPS) {
             ptx::mbar_wait(full0 + 8 * slot, par);
-            convert_x(slot, 0);
-        }
-        __syncwarp();
-        uint32_t it = 0;
-        for (int s = group; s < nstages; s += GV_GROUPS, ++it) {
-            const int cur = slot;                                     // full: waited for when its X was converted
-            const uint32_t base = ring + cur * GV_SLOT_BYTES + woff;
+            const uint32_t base = ring + slot * GV_SLOT_BYTES + woff;
             uint4 wv[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j)                               // column i + 16 j is 2048 bytes further
@@ -149,15 +150,9 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
                              : "=r"(wv[j].x), "=r"(wv[j].y), "=r"(wv[j].z), "=r"(wv[j].w)
                              : "r"(base + j * 2048));
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(empty0 + 8 * cur);       // the stage's words are in registers: free the slot
-#pragma unroll
-            for (int t = 0; t < GV_GROUPS; ++t)                        // advance GV_GROUPS stages round the ring
-                if (++slot == nslots) { slot = 0; par ^= 1; }
-            const bool more = s + GV_GROUPS < nstages;
-            const bool early = more && __all_sync(0xffffffffu, ptx::mbar_try_wait(full0 + 8 * slot, par));
-            if (early) convert_x(slot, (it + 1) & 1);
+            if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);      // weights are in registers: free the slot
 
-            const uint32_t xa = xs_half + (it & 1) * (GV_XCHUNK * 4);
+            const uint32_t xa = xs_addr + (uint32_t)(s * 8 + chunk) * (GV_XCHUNK * 4);
 #pragma unroll
             for (int p = 0; p < 4; ++p) {                              // k-pairs of the chunk
                 float4 xv[4];                                          // x[2p][0..7], x[2p+1][0..7]
@@ -182,14 +177,12 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
                     acc[j][3] = __ffma2_rn(w1b, make_float2(xv[3].z, xv[3].w), acc[j][3]);
                 }
             }
-            if (more && !early) {
-                ptx::mbar_wait(full0 + 8 * slot, par);
-                convert_x(slot, (it + 1) & 1);
-            }
-            __syncwarp();                                             // scratch: next buffer written, this one read by all lanes
+#pragma unroll
+            for (int t = 0; t < GV_GROUPS; ++t)                        // advance GV_GROUPS stages round the ring
+                if (++slot == nslots) { slot = 0; par ^= 1; }
         }
 
-        // ===== cross-warp reduction through shared memory (ring, barriers and scratch are dead now) =====
+        // ===== cross-warp reduction through shared memory (ring, barriers and xs are dead now) =====
         asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
         // red[set][(j * 4 + q) * 32 + i * 2 + e] holds the partial sum of column i + 16 j, batch row 2 q + e.
         float2 *red = reinterpret_cast<float2 *>(smem);
@@ -199,7 +192,6 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
 #pragma unroll
             for (int q = 0; q < 4; ++q) mine[(j * 4 + q) * 16] = acc[j][q];
         asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-        ptx::pdl_wait();                                              // Y may still be read by the preceding kernel
         for (int o = threadIdx.x; o < GV_M * GV_COLS / 2; o += GV_CTHREADS) {
             float2 sum = make_float2(0.f, 0.f);
 #pragma unroll
@@ -221,20 +213,20 @@ gemv_nk8_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
 
 // Enqueues the kernel above for up to 8 rows (x, y already offset to the first of them).  Returns a TRI_* status.
 int launch_gemv_nk8(int mr, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, uint16_t *y,
-                    int64_t ldy, const DeviceInfo *, cudaStream_t s)
+                    int64_t ldy, const DeviceInfo *di, cudaStream_t s)
 {
     using namespace g8;
-    CUtensorMap wmap, xmap;
+    CUtensorMap wmap;
     int st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
-    // X rows 0 .. mr - 1; the 8-row box is zero-filled beyond them and beyond k
-    st = make_tmap_2d_bf16(&xmap, x, (uint64_t)k, (uint64_t)mr, (uint64_t)ldx * 2, GV_STAGE_K, GV_M, CU_TENSOR_MAP_SWIZZLE_NONE);
-    if (st != TRI_OK) return st;
-    const int nslots = GV_MAX_SLOTS;
-    const size_t smem = gemv_smem_bytes(nslots);
+    const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+    int nslots = GV_MAX_SLOTS < nstages ? GV_MAX_SLOTS : nstages;       // deepest ring that fits beside xs
+    while (nslots > 2 && gemv_smem_bytes(nslots, nstages) > di->smem_optin) --nslots;
+    const size_t smem = gemv_smem_bytes(nslots, nstages);
+    if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
     static bool attr_set = false;
     if (!attr_set) {
-        TRI_CUDA(cudaFuncSetAttribute(gemv_nk8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        TRI_CUDA(cudaFuncSetAttribute(gemv_nk8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)di->smem_optin));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg = {};
@@ -247,7 +239,7 @@ int launch_gemv_nk8(int mr, int n, int k, const uint16_t *x, int64_t ldx, const 
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    TRI_CUDA(cudaLaunchKernelEx(&cfg, gemv_nk8_kernel, wmap, xmap, y, ldy, mr, n, k, nslots));
+    TRI_CUDA(cudaLaunchKernelEx(&cfg, gemv_nk8_kernel, wmap, x, ldx, y, ldy, mr, n, k, nslots));
     return TRI_OK;
 }
 
