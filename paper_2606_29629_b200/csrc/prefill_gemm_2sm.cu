@@ -2,7 +2,7 @@
 //
 // Why pairs: one 128 x 256 x 16 MMA reads 4 KiB of A and 8 KiB of B from shared memory in 128 cycles (96 B/clk) while
 // TMA writes the same 12 KiB per 128 cycles for the next stages — together more than the 128 B/clk a shared
-// memory delivers, and the single-CTA kernel stops at 79 % tensor-pipe activity (profiles/r1a).  With
+// memory delivers, and the single-CTA kernel stops at 79 % tensor-pipe activity (profiles/r1a_ncu_prefill_gemm.txt).  With
 // tcgen05.mma.cta_group::2 the two SMs of a TPC compute one 256 x 256 tile: each SM holds its own 128 rows of A
 // and only HALF of the W tile (128 of the 256 columns), the tensor cores of both read both halves, so every SM
 // stages and reads 8 KiB per MMA instead of 12.
