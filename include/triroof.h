@@ -196,6 +196,13 @@ int tri_nvml_sample(int device, tri_sample *out);
  * returns delta(clock64) / delta(globaltimer ns) * 1000 in *mhz.  Blocking (synchronises stream). */
 int tri_sm_clock_mhz(unsigned spin_us, double *mhz, void *stream);
 
+/* Machine probe: issue cost of the mixed-precision FMA (fma.rn.f32.bf16, SASS FHFMA.BF16) by operand
+ * pattern.  pattern 0: both bf16 operands repeat between consecutive FMAs (only the accumulator register is fetched);
+ * 1: one repeats and the two fetched registers have the same parity; 2: operands repeat only every other instruction.
+ * sm_mhz: the SM clock to convert time into cycles (read it with tri_sm_clock_mhz or NVML).  *cycles_per_fma: issue
+ * cycles per warp-level FMA on one SM sub-partition.  Blocking; allocates and frees 12 KiB of device memory. */
+int tri_probe_fma_issue(int pattern, double sm_mhz, double *cycles_per_fma, void *stream);
+
 /* ------------------------------------------------------------------------------------------------
  * f3. A.I.-aware frequency selection (section III-C): the throughput and power
  *     models the sweep data feed, and the Eq. 6 solver.  HOST functions: no GPU, no NVML; every pointer

@@ -40,7 +40,7 @@ EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "t
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
            "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_solve_clock",
-           "tri_fit_theta"]
+           "tri_fit_theta", "tri_probe_fma_issue"]
 
 
 class TriError(RuntimeError):
@@ -115,6 +115,7 @@ def lib():
     L.tri_reset_clocks.argtypes = [c_int]
     L.tri_nvml_sample.argtypes = [c_int, POINTER(tri_sample)]
     L.tri_sm_clock_mhz.argtypes = [c_uint, POINTER(c_double), c_void_p]
+    L.tri_probe_fma_issue.argtypes = [c_int, c_double, POINTER(c_double), c_void_p]
     for name in ("tri_model_theta", "tri_model_phi"):
         getattr(L, name).argtypes = [POINTER(tri_model), c_double, c_double]
         getattr(L, name).restype = c_double
@@ -325,3 +326,10 @@ def tri_fit_theta(ai, f_mhz, theta, ai_mem, ai_cmp, gamma=0.0):
     _check(lib().tri_fit_theta((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*theta), n, ai_mem, ai_cmp, gamma,
                                byref(m)), "tri_fit_theta")
     return {"eta": m.eta, "beta": m.beta, "omega": m.omega, "gamma": m.gamma}
+
+
+def tri_probe_fma_issue(pattern: int, sm_mhz: float, stream=None) -> float:
+    """Issue cycles per FHFMA.BF16 for operand pattern 0 / 1 / 2 (include/triroof.h)."""
+    v = c_double(0.0)
+    _check(lib().tri_probe_fma_issue(pattern, sm_mhz, byref(v), _stream(stream)), "tri_probe_fma_issue")
+    return v.value

@@ -22,6 +22,7 @@ int fail(int status, const char *fmt, ...)
 static std::mutex g_mu;
 static DeviceInfo g_info;
 static bool g_ready = false;
+static int g_generation = 0;
 static unsigned long long *g_clock_scratch = nullptr;
 
 static int init_locked(int device)
@@ -50,8 +51,11 @@ static int init_locked(int device)
     di.smem_optin = (size_t)v;
     g_info = di;
     g_ready = true;
+    ++g_generation;
     return TRI_OK;
 }
+
+int device_generation() { return g_generation; }
 
 int ensure_init(const DeviceInfo **info)
 {

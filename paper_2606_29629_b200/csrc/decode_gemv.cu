@@ -270,11 +270,11 @@ template <int MR, bool KN>
 static cudaError_t launch_gemv(const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int m, int n, int k,
                                int nslots, size_t smem, int blocks, cudaStream_t s)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen != device_generation()) {
         cudaError_t e = cudaFuncSetAttribute(gemv_kernel<MR, KN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS));
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        attr_gen = device_generation();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(blocks);

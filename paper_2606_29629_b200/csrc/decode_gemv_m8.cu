@@ -224,10 +224,10 @@ int launch_gemv_nk8(int mr, int n, int k, const uint16_t *x, int64_t ldx, const 
     while (nslots > 2 && gemv_smem_bytes(nslots, nstages) > di->smem_optin) --nslots;
     const size_t smem = gemv_smem_bytes(nslots, nstages);
     if (smem > di->smem_optin) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d needs %zu B of shared memory", k, smem);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemv_nk8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)di->smem_optin));
-        attr_set = true;
+        attr_gen = device_generation();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((n + GV_COLS - 1) / GV_COLS);

@@ -230,10 +230,10 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     if (st != TRI_OK) return st;
     if (!one_sm) return launch_gemm_2sm(amap, wmap, p, di->sm_count, static_cast<cudaStream_t>(stream));
 
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_BYTES));
-        attr_set = true;
+        attr_gen = device_generation();
     }
     const int ntiles = p.tiles_m * p.tiles_n;
     const int grid = ntiles < di->sm_count ? ntiles : di->sm_count;

@@ -184,10 +184,10 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
 
 int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const GemmParams &p, int sm_count, cudaStream_t s)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_2sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES));
-        attr_set = true;
+        attr_gen = device_generation();
     }
     const int ntiles = p.tiles_m * p.tiles_n;
     const int pairs = ntiles < sm_count / 2 ? ntiles : sm_count / 2;

@@ -20,6 +20,9 @@ struct DeviceInfo {
 // Sets the calling thread's detail text and returns `status` (so call sites can `return fail(...)`).
 int fail(int status, const char *fmt, ...) __attribute__((format(printf, 2, 3)));
 
+// Incremented every time the library (re)initialises on a device; kernels cache per-device function attributes against it.
+int device_generation();
+
 // Lazily initialises on the current device; returns TRI_OK or an error status.
 int ensure_init(const DeviceInfo **info);
 
