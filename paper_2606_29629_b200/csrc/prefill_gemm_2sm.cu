@@ -15,10 +15,10 @@
 //                           tcgen05.commit ... multicast arrives on "empty" (and, per tile, "tmem_full") in both CTAs
 //   warp 2   TMEM owner     tcgen05.alloc.cta_group::2 of all 512 columns = two 128 x 256 fp32 accumulators per
 //                           CTA, so the epilogue of tile t overlaps the main loop of tile t + 1
-//   warps 4-7 epilogue      tcgen05.ld of the CTA's own 128 rows -> bf16 RNE -> 16-byte stores; then arrive on the
-//                           LEADER's "tmem_empty" (8 arrivals: 4 warps x 2 CTAs)
+//   warps 4-7 epilogue      tcgen05.ld of the CTA's own 128 rows -> bf16 RNE -> swizzled shared-memory boxes -> TMA
+//                           stores (32 rows x 64 columns each); arrive on the LEADER's "tmem_empty" (8 arrivals)
 // 4096 x 18944 gives 16 x 74 = 1184 pair tiles = 74 TPCs x 16: no wave quantisation.  M index fastest, as in the
-// single-CTA kernel.  Ragged M / N / K: TMA zero fill, clipped stores.
+// single-CTA kernel.  Ragged M / N / K: TMA zero fill on loads, TMA clipping on stores (the last n % 8 columns are stored from registers).
 #include "tri_internal.h"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
@@ -33,18 +33,21 @@ constexpr int G2_B_BYTES = G2_BNH * G2_BK * 2;            // 16 KiB
 constexpr int G2_STAGE_BYTES = G2_A_BYTES + G2_B_BYTES;
 constexpr int G2_THREADS = 256;
 constexpr int G2_TMEM_COLS = 512;
-constexpr int G2_SMEM_BYTES = 1024 + G2_STAGES * G2_STAGE_BYTES + 256;
+constexpr int G2_OUT_BYTES = 4 * 2 * 4096;                 // epilogue staging: per warp two 32-row x 64-column bf16 boxes
+constexpr int G2_SMEM_BYTES = 1024 + G2_STAGES * G2_STAGE_BYTES + G2_OUT_BYTES + 256;
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(G2_THREADS, 1)
-gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap, const GemmParams p)
+gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap,
+                const __grid_constant__ CUtensorMap cmap, const GemmParams p)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const uint32_t ring = ptx::smem_u32(smem);
-    const uint32_t bars = ring + G2_STAGES * G2_STAGE_BYTES;
+    const uint32_t outbuf = ring + G2_STAGES * G2_STAGE_BYTES;        // 1 KiB aligned: 128-byte swizzle atoms
+    const uint32_t bars = outbuf + G2_OUT_BYTES;
     const uint32_t full0 = bars, empty0 = bars + 8 * G2_STAGES;
     const uint32_t tfull0 = bars + 16 * G2_STAGES, tempty0 = tfull0 + 16;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + G2_STAGES * G2_STAGE_BYTES + 16 * G2_STAGES + 32);
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + G2_STAGES * G2_STAGE_BYTES + G2_OUT_BYTES + 16 * G2_STAGES + 32);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = ptx::cluster_ctarank();
@@ -127,49 +130,68 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
             }
         }
     } else if (warp >= 4) {
-        // ===== epilogue (both CTAs): own 128 rows, TMEM -> registers -> bf16 -> global =====
+        // ===== epilogue (both CTAs): own 128 rows, TMEM -> registers -> bf16 -> shared memory -> TMA store =====
+        // A warp owns 32 rows.  Per 64-column group it packs its 32 x 64 bf16 box into one of its two 4 KiB staging
+        // buffers (row = 128 bytes, 16-byte chunks XOR-swizzled by row so the 8 lanes of a quarter-warp hit 8 bank
+        // groups) and one lane hands the box to TMA (cp.async.bulk.tensor store, 128-byte swizzle undone by the
+        // tensor map): full 128-byte lines to L2 instead of 32 half-sector writes per store instruction, ragged
+        // M / N clipped by TMA, and the warp is free again while the store drains.
         const int ew = warp & 3;                                      // TMEM lanes 32*ew .. 32*ew+31
-        uint32_t tcount = 0;
+        const uint32_t stage0 = outbuf + ew * 8192;
+        uint32_t tcount = 0, sb = 0;
+        if (lane == 0) ptx::prefetch_tmap(&cmap);
         for (int t = pair; t < ntiles; t += npairs, ++tcount) {
             const int tm = t % p.tiles_m, tn = t / p.tiles_m;
             const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
             ptx::mbar_wait(tfull0 + 8 * acc, aph);
             ptx::tc_fence_after();
-            const int row = tm * (2 * G2_BM) + (int)rank * G2_BM + ew * 32 + lane;
-            const bool row_ok = row < p.m;
-            uint16_t *crow = p.c + (int64_t)row * p.ldc + (int64_t)tn * G2_BN;
-            const int ncols = p.n - tn * G2_BN;                       // valid columns in this tile (may exceed 256)
+            const int row0 = tm * (2 * G2_BM) + (int)rank * G2_BM + ew * 32;
             const uint32_t taddr = tmem_base + acc * G2_BN + ((uint32_t)(ew * 32) << 16);
 #pragma unroll 1
-            for (int cb = 0; cb < G2_BN / 32; ++cb) {
-                uint32_t r[32];
-                ptx::tmem_ld_32x32b_x32(taddr + cb * 32, r);
-                ptx::tmem_ld_wait();
-                if (cb == G2_BN / 32 - 1) {                           // all TMEM reads of this tile are done
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive_cluster(tempty0 + 8 * acc, 0);
-                }
-                if (row_ok) {
+            for (int g = 0; g < G2_BN / 64; ++g, sb ^= 1) {
+                const uint32_t buf = stage0 + sb * 4096;
+                if (lane == 0) ptx::tma_store_wait_read<1>();         // the store that last read this buffer is done with it
+                __syncwarp();
 #pragma unroll
-                    for (int g = 0; g < 4; ++g) {                     // 8 columns = 16 bytes per store
-                        const int col = cb * 32 + g * 8;
-                        uint4 v;
-                        v.x = ptx::pack_bf16x2(__uint_as_float(r[g * 8 + 0]), __uint_as_float(r[g * 8 + 1]));
-                        v.y = ptx::pack_bf16x2(__uint_as_float(r[g * 8 + 2]), __uint_as_float(r[g * 8 + 3]));
-                        v.z = ptx::pack_bf16x2(__uint_as_float(r[g * 8 + 4]), __uint_as_float(r[g * 8 + 5]));
-                        v.w = ptx::pack_bf16x2(__uint_as_float(r[g * 8 + 6]), __uint_as_float(r[g * 8 + 7]));
-                        if (col + 8 <= ncols) {
-                            *reinterpret_cast<uint4 *>(crow + col) = v;
-                        } else if (col < ncols) {
-                            const uint32_t w4[4] = {v.x, v.y, v.z, v.w};
-                            for (int e = 0; e < 8 && col + e < ncols; ++e)
-                                crow[col + e] = (uint16_t)(w4[e >> 1] >> ((e & 1) * 16));
+                for (int h = 0; h < 2; ++h) {
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32b_x32(taddr + g * 64 + h * 32, r);
+                    ptx::tmem_ld_wait();
+                    if (g == G2_BN / 64 - 1 && h == 1) {              // all TMEM reads of this tile are done
+                        ptx::tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) ptx::mbar_arrive_cluster(tempty0 + 8 * acc, 0);
+                    }
+                    {   // TMA clips a partial box only at 16-byte granularity (measured: a box cut at column 257 also zeroes
+                        // columns 257..263), so the tensor map ends at n rounded down to 8 columns and the last n % 8 columns
+                        // are stored from registers here
+                        const int cbase = tn * G2_BN + g * 64 + h * 32, n8 = p.n & ~7, row = row0 + lane;
+                        if (cbase + 32 > n8 && cbase < p.n && row < p.m) {
+#pragma unroll
+                            for (int j = 0; j < 32; ++j)
+                                if (cbase + j >= n8 && cbase + j < p.n)
+                                    p.c[(int64_t)row * p.ldc + cbase + j] = (uint16_t)(ptx::pack_bf16x2(__uint_as_float(r[j]), 0.f) & 0xffffu);
                         }
                     }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {                     // 8 columns = one 16-byte chunk
+                        const uint32_t v0 = ptx::pack_bf16x2(__uint_as_float(r[q * 8 + 0]), __uint_as_float(r[q * 8 + 1]));
+                        const uint32_t v1 = ptx::pack_bf16x2(__uint_as_float(r[q * 8 + 2]), __uint_as_float(r[q * 8 + 3]));
+                        const uint32_t v2 = ptx::pack_bf16x2(__uint_as_float(r[q * 8 + 4]), __uint_as_float(r[q * 8 + 5]));
+                        const uint32_t v3 = ptx::pack_bf16x2(__uint_as_float(r[q * 8 + 6]), __uint_as_float(r[q * 8 + 7]));
+                        const uint32_t dst = buf + (uint32_t)lane * 128u + (uint32_t)(((h * 4 + q) ^ (lane & 7)) << 4);
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(v0), "r"(v1), "r"(v2), "r"(v3) : "memory");
+                    }
+                }
+                ptx::fence_proxy_async_smem();                        // generic-proxy writes visible to the TMA engine
+                __syncwarp();
+                if (lane == 0 && row0 < p.m && tn * G2_BN + g * 64 < (p.n & ~7)) {
+                    ptx::tma_store_2d(&cmap, buf, tn * G2_BN + g * 64, row0);
+                    ptx::tma_store_commit();
                 }
             }
         }
+        if (lane == 0) ptx::tma_store_wait<0>();                      // all of this warp's stores have landed
     }
 
     // Neither CTA may exit (or free TMEM) while the other can still read its shared memory or signal its barriers.
@@ -184,6 +206,10 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
 
 int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const GemmParams &p, int sm_count, cudaStream_t s)
 {
+    CUtensorMap cmap;     // C as 64-column x 32-row boxes for the epilogue's TMA stores (out-of-range rows / columns are clipped)
+    const int n8 = p.n & ~7;     // see the epilogue: the last n % 8 columns do not go through TMA
+    int st = make_tmap_2d_bf16(&cmap, p.c, (uint64_t)(n8 ? n8 : 8), (uint64_t)p.m, (uint64_t)p.ldc * 2, 64, 32, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (st != TRI_OK) return st;
     static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
     if (attr_gen != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_2sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES));
@@ -191,7 +217,7 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
     }
     const int ntiles = p.tiles_m * p.tiles_n;
     const int pairs = ntiles < sm_count / 2 ? ntiles : sm_count / 2;
-    gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, p);
+    gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, cmap, p);
     TRI_CUDA(cudaGetLastError());
     return TRI_OK;
 }

@@ -70,7 +70,7 @@ def test_ones_give_k_exactly(layout, k):
 
 @pytest.mark.parametrize("layout", LAYOUTS)
 @pytest.mark.parametrize("m,n,k", [(1, 8, 8), (7, 8, 80), (8, 264, 64), (9, 256, 72), (127, 257, 200), (128, 512, 128),
-                                   (129, 520, 136), (300, 1000, 1032), (1000, 70, 64), (257, 3000, 328)])
+                                   (129, 520, 136), (300, 1000, 1032), (1000, 70, 64), (257, 3000, 328), (33, 5, 16), (260, 12, 24), (513, 263, 8)])
 def test_small_and_ragged_full_output(layout, m, n, k):
     a = normal_bf16(60 + m % 7, (m, k))
     w = normal_bf16(61 + n % 7, (k, n), 0.05)
