@@ -292,6 +292,42 @@ def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
     return out
 
 
+def gemm_ai_series(torch, tri, peaks):
+    """Row f4 (next): the paper's own microbenchmark form — a matmul whose A.I. is varied — on the
+    tensor-core path: C[8192 x 8192] = A[8192 x K] W[K x 8192], bf16, K swept; A.I. = 2 m n K / (2 (m K + K n + m n)).
+    Roofline: min(measured cuBLAS burst, A.I. x measured HBM).  torch.matmul (cuBLAS) on the same operands is timed
+    beside it as context."""
+    m = n = 8192
+    out = []
+    for k in (16, 64, 256, 1024, 4096):
+        a = (torch.randn(m, k, device="cuda")).bfloat16()
+        w = (torch.randn(n, k, device="cuda") * 0.02).bfloat16()
+        c = torch.empty(m, n, device="cuda", dtype=torch.bfloat16)
+
+        def med(fn):
+            for _ in range(2):
+                fn()
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(9)]
+            for x, y in ev:
+                x.record()
+                fn()
+                y.record()
+            torch.cuda.synchronize()
+            return sorted(x.elapsed_time(y) for x, y in ev)[4]
+
+        ours = med(lambda: tri.prefill_gemm(m, n, k, a, k, w, k, tri.TRI_W_NK, c, n))
+        lib = med(lambda: torch.matmul(a, w.T, out=c))
+        flop, nbytes = 2.0 * m * n * k, 2.0 * (m * k + n * k + m * n)
+        ai = flop / nbytes
+        roof = min(peaks["bf16_tflops"], ai * peaks["hbm_gbs"] / 1e3)
+        out.append({"kernel": "prefill_gemm", "series": "matmul-based A.I. sweep (PAPER.md line 92), 8192 x 8192 x K", "k": k, "ai": ai,
+                    "ms": ours, "tflops": flop / ours / 1e9, "gbs": nbytes / ours / 1e6, "roofline_tflops": roof,
+                    "frac": flop / ours / 1e9 / roof, "bound": "tensor" if roof == peaks["bf16_tflops"] else "hbm",
+                    "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9})
+        del a, w, c
+    return out
+
+
 def run_ours(args):
     import torch
     import paper_2606_29629_b200 as tri          # raises if the CUDA library cannot be built / loaded: no fallback
@@ -408,6 +444,7 @@ def run_ours(args):
                                  source="PAPER.md Eq. 4 via tri_fit_theta on the sustained sweep points (memory set A.I. <= 4, compute set A.I. >= 32)")
             except tri.TriError as e:
                 model_fit = {"error": str(e)}
+        extra_points += gemm_ai_series(torch, tri, peaks)
         for kk in PAPER_KS:                                            # the paper's x-axis (Fig. 3), labelled extra series
             c = ch.get(f"paper_ai{kk / 4:g}")
             if c:

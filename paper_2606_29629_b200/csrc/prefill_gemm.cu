@@ -216,6 +216,11 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     p.kblocks = (k + GM_BK - 1) / GM_BK;
     p.ldc = ldc;
     p.c = c;
+    {
+        static int wpol = -1;                               // debug only: TRI_GEMM_WPOL in {0, 1, 2}
+        if (wpol < 0) { const char *e = getenv("TRI_GEMM_WPOL"); wpol = e ? atoi(e) : 2; }      // measured on config 4: evict-last 1.392 PFLOP/s sustained, evict-first 1.374
+        p.w_policy = wpol;
+    }
     if (w_layout == TRI_W_NK) {
         st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, bn_box, CU_TENSOR_MAP_SWIZZLE_128B);
         p.b_mn_major = 0;
