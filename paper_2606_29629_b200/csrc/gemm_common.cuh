@@ -31,6 +31,7 @@ struct GemmParams {
     int b_mn_major;          // 0: W is [n][k] (K-major);  1: W is [k][n] (MN-major)
     uint32_t b_lbo, b_sbo;   // descriptor strides of the B operand
     uint32_t b_kstep;        // byte advance of the B start address per UMMA_K = 16
+    int group_m;             // CTA-pair kernel: row blocks per tile group (see tile_coords)
     int w_policy;            // L2 policy of the W loads: 0 evict-first, 1 evict-normal, 2 evict-last
 };
 

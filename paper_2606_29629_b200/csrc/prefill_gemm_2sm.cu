@@ -36,6 +36,17 @@ constexpr int G2_TMEM_COLS = 512;
 constexpr int G2_OUT_BYTES = 4 * 2 * 4096;                 // epilogue staging: per warp two 32-row x 64-column bf16 boxes
 constexpr int G2_SMEM_BYTES = 1024 + G2_STAGES * G2_STAGE_BYTES + G2_OUT_BYTES + 256;
 
+// Tile order: M index fastest inside groups of p.group_m row blocks, groups one after the other.  A group's A panels
+// (group_m x 256 rows x K) stay L2-resident while the W panels stream past once per group; group_m = all row blocks
+// when A fits (config 4: 29 MB), smaller for tall A so that the resident set stays near 32 MB.
+__device__ __forceinline__ void tile_coords(const GemmParams &p, int t, int &tm, int &tn)
+{
+    const int per_group = p.group_m * p.tiles_n, grp = t / per_group, r = t - grp * per_group;
+    const int m0 = grp * p.group_m, gm = (p.tiles_m - m0 < p.group_m) ? p.tiles_m - m0 : p.group_m;
+    tm = m0 + r % gm;
+    tn = r / gm;
+}
+
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(G2_THREADS, 1)
 gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap,
                 const __grid_constant__ CUtensorMap cmap, const GemmParams p)
@@ -87,7 +98,8 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
             const uint64_t pol_a = ptx::policy_evict_last();
             uint32_t it = 0;
             for (int t = pair; t < ntiles; t += npairs) {
-                const int tm = t % p.tiles_m, tn = t / p.tiles_m;
+                int tm, tn;
+            tile_coords(p, t, tm, tn);
                 const int row0 = tm * (2 * G2_BM) + (int)rank * G2_BM, col0 = tn * G2_BN + (int)rank * G2_BNH;
                 for (int kb = 0; kb < p.kblocks; ++kb, ++it) {
                     const uint32_t s = it % G2_STAGES, ph = (it / G2_STAGES) & 1;
@@ -144,7 +156,8 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         uint32_t tcount = 0, sb = 0;
         if (lane == 0) ptx::prefetch_tmap(&cmap);
         for (int t = pair; t < ntiles; t += npairs, ++tcount) {
-            const int tm = t % p.tiles_m, tn = t / p.tiles_m;
+            int tm, tn;
+            tile_coords(p, t, tm, tn);
             const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
             ptx::mbar_wait(tfull0 + 8 * acc, aph);
             ptx::tc_fence_after();
@@ -220,7 +233,14 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
     }
     const int ntiles = p.tiles_m * p.tiles_n;
     const int pairs = ntiles < sm_count / 2 ? ntiles : sm_count / 2;
-    gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, cmap, p);
+    GemmParams q = p;
+    {   // rows of A kept resident: about 32 MB worth of 256-row panels, at least 4, all of them when A is small
+        const double panel = 256.0 * p.k * 2.0;
+        int g = (int)(32.0e6 / panel);
+        g = g < 4 ? 4 : g;
+        q.group_m = g < p.tiles_m ? g : p.tiles_m;
+    }
+    gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, cmap, q);
     TRI_CUDA(cudaGetLastError());
     return TRI_OK;
 }
