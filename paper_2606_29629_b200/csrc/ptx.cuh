@@ -161,13 +161,15 @@ __device__ __forceinline__ void cluster_sync()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
-// Arrive on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster.
+// Arrive on the mbarrier at the same shared-memory offset in CTA `rank` of the cluster (default .release.cta semantics:
+// a cluster-scope release costs a MEMBAR + ERRBAR per arrive; what the waiter consumes here is TMEM, ordered by the
+// tcgen05 fences on both sides).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank)
 {
     asm volatile(
         "{\n\t.reg .b32 ra;\n\t"
         "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
-        "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}"
+        "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}"
         ::"r"(bar), "r"(rank)
         : "memory");
 }
