@@ -305,7 +305,7 @@ def gemm_ai_series(torch, tri, peaks):
         c = torch.empty(m, n, device="cuda", dtype=torch.bfloat16)
 
         def med(fn):
-            for _ in range(2):
+            for _ in range(20):                                           # the part idles between points: let the clocks come back
                 fn()
             ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(9)]
             for x, y in ev:
