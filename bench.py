@@ -33,6 +33,8 @@ GEMV_SHAPE = (8, 18944, 3584)         # m, n, k
 GEMM_SHAPE = (4096, 18944, 3584)
 GEMV_COPIES = 8
 PAPER_KS = [4, 100, 200, 400, 800]      # the paper's own A.I. set {1, 25, 50, 100, 200} FLOP/B
+NOMINAL_HBM_GBS = 8000.0               # BASELINE.json north_star "roughly 8 TB/s" (context; `frac` uses the measured peaks)
+NOMINAL_BF16_TFLOPS = 2250.0           # dense bf16, nominal
 FP32_LANES_PER_SM = 128                # FP32 FMA lanes per SM (4 SMSPs x 32); DESIGN.md "ALU peak"
 REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
            0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
@@ -391,17 +393,20 @@ def run_ours(args):
         roof = min(alu_peak, k / 4.0 * peaks["hbm_gbs"] / 1e3)
         points.append({"kernel": "fma_chain", "k": k, "ai": k / 4.0, "ms": ms, "gbs": gbs, "tflops": tf,
                        "bound": "hbm" if k / 4.0 * peaks["hbm_gbs"] / 1e3 < alu_peak else "alu",
-                       "roofline_tflops": roof, "frac": tf / roof})
+                       "roofline_tflops": roof, "frac": tf / roof, "ms_min": min(per[f"fma_k{k}"]),
+                       "frac_vs_nominal": tf / min(alu_peak, k / 4.0 * NOMINAL_HBM_GBS / 1e3)})
     ms = statistics.median(per["gemv"]) / GEMV_COPIES
     gv_gbs = gemm_bytes(GEMV_SHAPE) / ms / 1e6
     points.append({"kernel": "decode_gemv", "ai": gemm_flop(GEMV_SHAPE) / gemm_bytes(GEMV_SHAPE), "ms": ms, "gbs": gv_gbs,
                    "tflops": gemm_flop(GEMV_SHAPE) / ms / 1e9, "bound": "hbm", "roofline_gbs": peaks["hbm_gbs"],
-                   "frac": gv_gbs / peaks["hbm_gbs"]})
+                   "frac": gv_gbs / peaks["hbm_gbs"], "ms_min": min(per["gemv"]) / GEMV_COPIES,
+                   "frac_vs_nominal": gv_gbs / NOMINAL_HBM_GBS})
     ms = statistics.median(per["gemm"])
     gm_tf = gemm_flop(GEMM_SHAPE) / ms / 1e9
     points.append({"kernel": "prefill_gemm", "ai": gemm_flop(GEMM_SHAPE) / gemm_bytes(GEMM_SHAPE), "ms": ms,
                    "gbs": gemm_bytes(GEMM_SHAPE) / ms / 1e6, "tflops": gm_tf, "bound": "tensor",
-                   "roofline_tflops": peaks["bf16_tflops"], "frac": gm_tf / peaks["bf16_tflops"]})
+                   "roofline_tflops": peaks["bf16_tflops"], "frac": gm_tf / peaks["bf16_tflops"], "ms_min": min(per["gemm"]),
+                   "frac_vs_nominal": gm_tf / NOMINAL_BF16_TFLOPS})
 
     # ---- per-point sustained pass: clock, temperature, power, J/op per A.I. point and per phase kernel ----
     extra_points, model_fit = [], None
