@@ -66,6 +66,19 @@ def test_config3_full_output(layout):
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
+@pytest.mark.parametrize("m", [1, 4, 5, 16])
+def test_config3_shape_other_batch_sizes(layout, m):
+    """The config-3 weight matrix at the other decode batch sizes: m = 1, 4 run the FHFMA kernel in
+    both layouts, m = 5 the FFMA2 kernel with zero-filled rows, m = 16 two launches of 8 rows; full output, stated bound."""
+    k, n = 3584, 18944
+    x = normal_bf16(2, (m, k), 1.0, stream=7)
+    w = normal_bf16(2, (k, n), 0.02, stream=1)
+    wp = phys_w(w, layout)
+    y = run_gemv(x, wp, m, n, k, layout)
+    assert check_against_oracle(y, x, wp, layout, stated=True) < 1.0
+
+
+@pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
 def test_identity_and_permutation_are_exact(layout):
     k = n = 256
     x = normal_bf16(21, (8, k))
