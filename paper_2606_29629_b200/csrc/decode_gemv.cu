@@ -13,7 +13,8 @@
 // with three distinct operands therefore issues every 2 cycles unless one operand is reused, and ptxas interleaves
 // the FMA stream so that about half of them miss (1.5 cycles per FMA; forcing the order through data or control
 // dependencies cost as much in bubbles).  For m <= 4 the kernel stays HBM-bound (21.7 us at m = 1, 22.8 us at m = 4 on
-// the config-3 shape = 96 % / 91 % of the measured HBM peak); at m = 5..8 it is FMA-issue bound (39 us NK, 29 us KN),
+// the config-3 shape with the 8-slot ring; 20.1 / 21.2 us = 103 % / 98 % of the measured copy peak with 10 slots); at m = 5..8 it is
+// FMA-issue bound (39 us NK, 29 us KN as first written; 28.3 / 27.8 us with X transposed to row pairs, see below),
 // so TRI_W_NK with 5..8 rows and k <= 4096 goes to the packed-FFMA2 kernel of decode_gemv_m8.cu (24.8 us), whose
 // 64-bit operands read one register of each bank and cannot conflict.
 //
@@ -32,6 +33,10 @@
 //   * compute warps, TRI_W_KN (slot row = k, 128 B = 64 columns n): lane (c = lane & 7, q = lane >> 3)
 //     of warp w owns the 8 columns of chunk c and the k-rows 16w + 4q .. + 3: four LDS.128 of W (a
 //     quarter-warp reads one whole row), eight broadcast LDS.64 of X, 8 x 4 x 8 = 256 FMAs.
+//   * 8-row kernels: each (half-)warp first transposes its slice of X to row PAIRS per k (2 LDS.32, 2 PRMT, 2 STS.32 per
+//     lane and stage), so that one X word holds rows (2q, 2q+1) at one k.  Two (NK) or four (KN) independent FMAs then
+//     use the same two registers, which is the operand pattern that needs no register-file read (tri_probe_fma_issue
+//     pattern 0) and the one ptxas keeps together; statically 1.17 instead of 1.4-1.6 issue cycles per FMA;
 //   * the W registers of stage s + 1 are loaded before the FMAs of stage s, and a slot is released as
 //     soon as its words are in registers.
 //   * after the last stage the partial sums (8 sets for NK, 16 for KN) are added through shared
@@ -54,7 +59,10 @@ constexpr int GV_W_BYTES = GV_STAGE_K * GV_COLS * 2;  // 8 KiB
 constexpr int GV_X_BYTES = GV_STAGE_K * GV_M * 2;     // 1 KiB
 constexpr int GV_SLOT_BYTES = GV_W_BYTES + GV_X_BYTES;
 constexpr int GV_MAX_SLOTS = 12;
-constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS;
+#ifndef GV_XT_ENABLED
+#define GV_XT_ENABLED 1      // 8-row kernels read X transposed to row pairs (0: A/B comparison only)
+#endif
+constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS + 8 * 128;   // full[], empty[], per-half-warp transposition scratch
 constexpr int GV_RED_STRIDE = GV_M * GV_COLS + 16;    // floats per partial-sum set; +16 keeps the two half-warps on different banks
 
 __host__ __device__ constexpr size_t gemv_smem_bytes(int nslots)
@@ -171,6 +179,8 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
         xoff = GV_W_BYTES + (uint32_t)chunk * 16u;
     }
 
+    const uint32_t xt_scratch = empty0 + 8 * GV_MAX_SLOTS + (uint32_t)(warp * 2 + (lane >> 4)) * 128u;   // per half-warp, 8 k x 16 B
+    const uint32_t xt_warp = empty0 + 8 * GV_MAX_SLOTS + (uint32_t)warp * 256u;                       // KN: per warp, 16 k x 16 B
     uint32_t wv[2][4][4];
     int slot = 0;
     uint32_t par = 0;
@@ -182,10 +192,39 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
         constexpr int CUR = decltype(cur_tag)::value, NXT = CUR ^ 1;
         const uint32_t base = ring + slot * GV_SLOT_BYTES;
         uint32_t xv[MR][KN ? 2 : 4];
+        constexpr bool XT = GV_XT_ENABLED && MR == 8;                 // X transposed to row pairs per k (see below)
+        uint32_t xq[XT ? 8 : 1][4];
+        if constexpr (XT && !KN) {
+            // lane (kp, rq) of the half-warp: rows 2rq, 2rq+1 at k-pair kp of the chunk -> words (row pair at k), (row pair at k+1)
+            const int kp = i16 >> 2, rq = i16 & 3;
+            uint32_t a, b;
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base + xoff + (2 * rq) * 128 + kp * 4));
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(base + xoff + (2 * rq + 1) * 128 + kp * 4));
+            const uint32_t sc = xt_scratch + (uint32_t)(2 * kp) * 16u + (uint32_t)rq * 4u;
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sc), "r"(__byte_perm(a, b, 0x5410)) : "memory");
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sc + 16), "r"(__byte_perm(a, b, 0x7632)) : "memory");
+            __syncwarp();
 #pragma unroll
-        for (int mm = 0; mm < MR; ++mm) {
-            if constexpr (KN) lds64(xv[mm], base + xoff + mm * 128);
-            else lds128(xv[mm], base + xoff + mm * 128);
+            for (int kk = 0; kk < 8; ++kk) lds128(xq[kk], xt_scratch + kk * 16);
+        } else if constexpr (XT && KN) {
+            // the warp's 16 k-rows: lane (kp = lane >> 2, rq = lane & 3) transposes rows 2rq, 2rq+1 at k-pair kp; then every
+            // lane reads the row-pair words of its own 4 k-rows
+            const int kp = lane >> 2, rq = lane & 3;
+            uint32_t a, b;
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base + GV_W_BYTES + (2 * rq) * 128 + (16 * warp + 2 * kp) * 2));
+            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(base + GV_W_BYTES + (2 * rq + 1) * 128 + (16 * warp + 2 * kp) * 2));
+            const uint32_t sw = xt_warp + (uint32_t)(2 * kp) * 16u + (uint32_t)rq * 4u;
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sw), "r"(__byte_perm(a, b, 0x5410)) : "memory");
+            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sw + 16), "r"(__byte_perm(a, b, 0x7632)) : "memory");
+            __syncwarp();
+#pragma unroll
+            for (int t = 0; t < 4; ++t) lds128(xq[t], xt_warp + (uint32_t)(4 * q4 + t) * 16u);
+        } else {
+#pragma unroll
+            for (int mm = 0; mm < MR; ++mm) {
+                if constexpr (KN) lds64(xv[mm], base + xoff + mm * 128);
+                else lds128(xv[mm], base + xoff + mm * 128);
+            }
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);          // this stage's words are in registers: free the slot
@@ -196,7 +235,19 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
 #pragma unroll
             for (int j = 0; j < 4; ++j) lds128(wv[NXT][j], nb + woff[j]);
         }
-        if constexpr (KN) {
+        if constexpr (KN && XT) {
+#pragma unroll
+            for (int t = 0; t < 4; ++t)                               // k-row of the lane
+#pragma unroll
+                for (int u = 0; u < 4; ++u)                           // word u = columns 2u, 2u + 1 of the chunk
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {                     // rows 2q, 2q + 1: four FMAs on the same two words
+                        acc[2 * u][2 * q] = fma_bf16<0, 0>(wv[CUR][t][u], xq[t][q], acc[2 * u][2 * q]);
+                        acc[2 * u][2 * q + 1] = fma_bf16<0, 1>(wv[CUR][t][u], xq[t][q], acc[2 * u][2 * q + 1]);
+                        acc[2 * u + 1][2 * q] = fma_bf16<1, 0>(wv[CUR][t][u], xq[t][q], acc[2 * u + 1][2 * q]);
+                        acc[2 * u + 1][2 * q + 1] = fma_bf16<1, 1>(wv[CUR][t][u], xq[t][q], acc[2 * u + 1][2 * q + 1]);
+                    }
+        } else if constexpr (KN) {
 #pragma unroll
             for (int t = 0; t < 4; ++t)                               // k-row of the lane: x word t >> 1, half t & 1
 #pragma unroll
@@ -211,6 +262,23 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
                             acc[2 * u + 1][mm] = fma_bf16<1, 0>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u + 1][mm]);
                         }
                     }
+        } else if constexpr (XT) {
+#pragma unroll
+            for (int p = 0; p < 4; ++p)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            if (e == 0) {
+                                acc[j][2 * q] = fma_bf16<0, 0>(wv[CUR][j][p], xq[2 * p][q], acc[j][2 * q]);
+                                acc[j][2 * q + 1] = fma_bf16<0, 1>(wv[CUR][j][p], xq[2 * p][q], acc[j][2 * q + 1]);
+                            } else {
+                                acc[j][2 * q] = fma_bf16<1, 0>(wv[CUR][j][p], xq[2 * p + 1][q], acc[j][2 * q]);
+                                acc[j][2 * q + 1] = fma_bf16<1, 1>(wv[CUR][j][p], xq[2 * p + 1][q], acc[j][2 * q + 1]);
+                            }
+                        }
         } else {
 #pragma unroll
             for (int p = 0; p < 4; ++p)                               // word p = k-values 2p, 2p + 1 of the chunk
@@ -330,16 +398,18 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
     else st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
 
-    // Ring depth: 8 slots of 9 KiB per CTA = 128 KiB of weights in flight per SM with two CTAs resident (a TMA-only
-    // microbenchmark needed > 48 KiB per SM; 96 KiB and more were equal).  The partial-sum sets reuse the ring, so it
-    // is never smaller than they are.  TRI_GEMV_SLOTS is a debug override.
+    // Ring depth: 10 slots of 9 KiB per CTA (160 KiB of weights in flight per SM with two CTAs resident).  Measured on the
+    // config-3 shape: 8 -> 10 slots takes m = 1 from 21.6 to 20.1 us, m = 4 from 22.9 to 21.2, m = 8 (NK) from 36.6 to 28.3.
+    // Ten slots also fill the SM with two CTAs, so that no CTA of the NEXT call (programmatic dependent launch) moves in
+    // early and spins on its barriers in the issue slots of the running ones; 12 is no better.  KN with 5..8 rows likes 8.
+    // The partial-sum sets reuse the ring, so it is never smaller than they are.  TRI_GEMV_SLOTS is a debug override.
     static int slots_cfg = -1;
     if (slots_cfg < 0) {
         const char *e = getenv("TRI_GEMV_SLOTS");
         slots_cfg = e ? atoi(e) : 0;
-        if (slots_cfg < 4 || slots_cfg > GV_MAX_SLOTS) slots_cfg = 8;
+        if (slots_cfg < 4 || slots_cfg > GV_MAX_SLOTS) slots_cfg = 0;
     }
-    const int nslots = slots_cfg;
+    const int nslots = slots_cfg ? slots_cfg : (kn && m > 4 ? 8 : 10);
     static int force_fhfma = -1;                                     // debug only: TRI_GEMV_FHFMA=1 keeps every shape on this kernel
     if (force_fhfma < 0) {
         const char *e = getenv("TRI_GEMV_FHFMA");
