@@ -447,6 +447,18 @@ def run_ours(args):
                                  eta_nominal=sms * FP32_LANES_PER_SM * 2 / 1e6, beta_measured_copy=peaks["hbm_gbs"] / 1e3,
                                  max_abs_rel_residual=max(abs(r) for r in res), rel_residuals=[round(r, 4) for r in res],
                                  source="PAPER.md Eq. 4 via tri_fit_theta on the sustained sweep points (memory set A.I. <= 4, compute set A.I. >= 32)")
+                # Eq. 2 at the one clock this box shows below the cap (the boost ceiling): P_idle(f), P_dyn(f) from the
+                # compute-bound points that ran there
+                allp = [(pt["ai"], pt["sustained"]["sm_mhz"], pt["sustained"]["power_w_mean"]) for pt in points + extra_points
+                        if pt["kernel"] == "fma_chain" and pt.get("sustained") and pt["sustained"].get("sm_mhz")
+                        and pt["sustained"].get("power_w_mean")]
+                try:
+                    pf = tri.tri_fit_power([x[0] for x in allp], [x[1] for x in allp], [x[2] for x in allp], fit["eta"], fit["beta"],
+                                           peaks["sm_max_mhz"], 2.0, 950.0)
+                    model_fit["power_at_max_clock"] = dict(pf, f_mhz=peaks["sm_max_mhz"],
+                                                           source="PAPER.md Eq. 2-3 via tri_fit_power on the points at the boost ceiling, below the power cap")
+                except tri.TriError as e:
+                    model_fit["power_at_max_clock"] = {"error": str(e)}
             except tri.TriError as e:
                 model_fit = {"error": str(e)}
         extra_points += gemm_ai_series(torch, tri, peaks)

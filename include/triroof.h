@@ -244,6 +244,12 @@ int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double ep
  * is not positive and finite. */
 int tri_fit_theta(const double *ai, const double *f_mhz, const double *theta, size_t n, double ai_mem, double ai_cmp,
                   double gamma, tri_model *m);
+/* Fit of Eq. 2 at ONE clock: among the n measured points (ai_i, f_i, p_i) those with |f_i - f_sel_mhz| <= f_tol_mhz and
+ * p_i < p_cap_w (not limited by the cap) give P_idle(f_sel) and P_dyn(f_sel) as intercept and slope of the ordinary
+ * least-squares line of p against phi(ai_i, f_i) (Eq. 3 with m->eta, m->beta).  TRI_ERR_INVALID_ARG with fewer than 2
+ * distinct abscissae or non-finite input.  *n_used (optional) returns how many points qualified. */
+int tri_fit_power(const double *ai, const double *f_mhz, const double *p_w, size_t n, const tri_model *m, double f_sel_mhz,
+                  double f_tol_mhz, double p_cap_w, double *p_idle_w, double *p_dyn_w, size_t *n_used);
 
 #ifdef __cplusplus
 }

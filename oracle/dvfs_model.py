@@ -60,3 +60,12 @@ def fit_theta(ai, f, th, ai_mem, ai_cmp, gamma):
     if slope < 0:
         slope, icpt = 0.0, float(np.mean(f[cmp_] / th[cmp_]))
     return {"eta": 1.0 / icpt, "beta": beta, "omega": slope / icpt, "gamma": gamma}
+
+
+def fit_power(ai, f, p, eta, beta, f_sel, f_tol, p_cap):
+    """Eq. 2 at one clock: numpy.polyfit of p against phi over the points at that clock and below the cap."""
+    ai, f, p = (np.asarray(v, dtype=np.float64) for v in (ai, f, p))
+    sel = (np.abs(f - f_sel) <= f_tol) & (p < p_cap)
+    x = np.array([phi(a, ff, eta, beta) for a, ff in zip(ai[sel], f[sel])])
+    slope, icpt = np.polyfit(x, p[sel], 1)
+    return {"p_idle_w": float(icpt), "p_dyn_w": float(slope), "n_used": int(sel.sum())}

@@ -40,7 +40,7 @@ EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "t
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
            "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_solve_clock",
-           "tri_fit_theta", "tri_probe_fma_issue"]
+           "tri_fit_theta", "tri_fit_power", "tri_probe_fma_issue"]
 
 
 class TriError(RuntimeError):
@@ -115,6 +115,8 @@ def lib():
     L.tri_reset_clocks.argtypes = [c_int]
     L.tri_nvml_sample.argtypes = [c_int, POINTER(tri_sample)]
     L.tri_sm_clock_mhz.argtypes = [c_uint, POINTER(c_double), c_void_p]
+    L.tri_fit_power.argtypes = [POINTER(c_double), POINTER(c_double), POINTER(c_double), c_size_t, POINTER(tri_model), c_double, c_double,
+                                c_double, POINTER(c_double), POINTER(c_double), POINTER(c_size_t)]
     L.tri_probe_fma_issue.argtypes = [c_int, c_double, POINTER(c_double), c_void_p]
     for name in ("tri_model_theta", "tri_model_phi"):
         getattr(L, name).argtypes = [POINTER(tri_model), c_double, c_double]
@@ -333,3 +335,13 @@ def tri_probe_fma_issue(pattern: int, sm_mhz: float, stream=None) -> float:
     v = c_double(0.0)
     _check(lib().tri_probe_fma_issue(pattern, sm_mhz, byref(v), _stream(stream)), "tri_probe_fma_issue")
     return v.value
+
+
+def tri_fit_power(ai, f_mhz, p_w, eta, beta, f_sel_mhz, f_tol_mhz, p_cap_w):
+    """Eq. 2 at one clock -> dict(p_idle_w, p_dyn_w, n_used)."""
+    n = len(ai)
+    m = Model(eta, beta)
+    pi, pd, used = c_double(0.0), c_double(0.0), c_size_t(0)
+    _check(lib().tri_fit_power((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*p_w), n, byref(m.c), f_sel_mhz, f_tol_mhz,
+                               p_cap_w, byref(pi), byref(pd), byref(used)), "tri_fit_power")
+    return {"p_idle_w": pi.value, "p_dyn_w": pd.value, "n_used": used.value}

@@ -152,4 +152,27 @@ int tri_fit_theta(const double *ai, const double *f_mhz, const double *th, size_
     return TRI_OK;
 }
 
+int tri_fit_power(const double *ai, const double *f_mhz, const double *p_w, size_t n, const tri_model *m, double f_sel_mhz,
+                  double f_tol_mhz, double p_cap_w, double *p_idle_w, double *p_dyn_w, size_t *n_used)
+{
+    int st = tri::check_model(m, false);
+    if (st != TRI_OK) return st;
+    if (!ai || !f_mhz || !p_w || !p_idle_w || !p_dyn_w || !tri::pos(f_sel_mhz) || !(f_tol_mhz >= 0.0) || !tri::pos(p_cap_w))
+        return tri::fail(TRI_ERR_INVALID_ARG, "NULL argument, or f_sel / p_cap not positive, or f_tol negative");
+    size_t k = 0;
+    double sx = 0.0, sy = 0.0, sxx = 0.0, sxy = 0.0;
+    for (size_t i = 0; i < n; ++i) {
+        if (!tri::pos(ai[i]) || !tri::pos(f_mhz[i]) || !std::isfinite(p_w[i])) return tri::fail(TRI_ERR_INVALID_ARG, "point %zu is not finite / positive", i);
+        if (std::fabs(f_mhz[i] - f_sel_mhz) > f_tol_mhz || !(p_w[i] < p_cap_w)) continue;
+        const double x = tri::phi(m, ai[i], f_mhz[i]);
+        sx += x; sy += p_w[i]; sxx += x * x; sxy += x * p_w[i]; ++k;
+    }
+    if (n_used) *n_used = k;
+    const double det = (double)k * sxx - sx * sx;
+    if (k < 2 || !(det > 1e-12 * (1.0 + (double)k * sxx))) return tri::fail(TRI_ERR_INVALID_ARG, "%zu usable points: the line is not determined", k);
+    *p_dyn_w = ((double)k * sxy - sx * sy) / det;
+    *p_idle_w = (sy - *p_dyn_w * sx) / (double)k;
+    return TRI_OK;
+}
+
 }  // extern "C"

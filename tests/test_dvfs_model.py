@@ -92,3 +92,21 @@ def test_fit_matches_oracle_on_noisy_sweep():
         assert got[key] == pytest.approx(want[key], rel=1e-7, abs=1e-12), key
     with pytest.raises(tri.TriError):
         tri.tri_fit_theta([1.0, 2.0], [1000.0, 1000.0], [1.0, 2.0], ai_mem=4.0, ai_cmp=32.0)
+
+
+def test_power_fit_matches_oracle_and_recovers_planted_line():
+    rng = np.random.default_rng(16)
+    eta, beta = 0.0379, 6.87
+    ai = np.array([0.25, 1, 4, 8, 16, 24, 32, 50, 64, 100, 128, 200, 256, 512, 1024], float)
+    f = np.where(ai < 20, rng.uniform(1550.0, 1800.0, ai.size), 1965.0)               # auto-boost: only the compute-bound end at 1965
+    p_true = np.array([min(480.0 + 770.0 * o.phi(a, x, eta, beta), 1000.0) for a, x in zip(ai, f)])
+    got = tri.tri_fit_power(list(ai), list(f), list(p_true), eta, beta, 1965.0, 1.0, 990.0)
+    assert got["n_used"] == int((ai >= 20).sum())
+    assert got["p_idle_w"] == pytest.approx(480.0, rel=1e-9) and got["p_dyn_w"] == pytest.approx(770.0, rel=1e-9)
+    noisy = p_true * rng.uniform(0.98, 1.02, ai.size)
+    got = tri.tri_fit_power(list(ai), list(f), list(noisy), eta, beta, 1965.0, 1.0, 990.0)
+    want = o.fit_power(ai, f, noisy, eta, beta, 1965.0, 1.0, 990.0)
+    for key in ("p_idle_w", "p_dyn_w", "n_used"):
+        assert got[key] == pytest.approx(want[key], rel=1e-8), key
+    with pytest.raises(tri.TriError):
+        tri.tri_fit_power(list(ai), list(f), list(noisy), eta, beta, 1000.0, 1.0, 990.0)      # no point at that clock
