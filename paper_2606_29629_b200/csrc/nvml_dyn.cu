@@ -109,7 +109,7 @@ void unload()
     g_tried = false;
 }
 
-int read_sample(const Api *a, Device h, tri_sample *s)
+int read_sample(const Api *a, Device h, tri_sample *s, bool with_energy)
 {
     unsigned v = 0;
     unsigned long long e = 0;
@@ -117,7 +117,7 @@ int read_sample(const Api *a, Device h, tri_sample *s)
     s->mem_mhz = (a->clock_info(h, CLOCK_MEM, &v) == SUCCESS) ? v : 0;
     s->temp_c = (a->temperature(h, TEMPERATURE_GPU, &v) == SUCCESS) ? v : 0;
     s->power_w = (a->power_usage(h, &v) == SUCCESS) ? (float)v * 1e-3f : 0.f;
-    s->energy_mj = (a->total_energy && a->total_energy(h, &e) == SUCCESS) ? e : 0;
+    if (with_energy) s->energy_mj = (a->total_energy && a->total_energy(h, &e) == SUCCESS) ? e : 0;
     s->clk_event_reasons = (a->clock_reasons && a->clock_reasons(h, &e) == SUCCESS) ? e : 0;
     return TRI_OK;
 }

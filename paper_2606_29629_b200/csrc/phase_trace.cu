@@ -43,6 +43,7 @@ struct Tracer {
     bool overflow = false;
     unsigned period_us = 10000;
     double t0 = 0.0;
+    uint64_t last_energy_mj = 0;
     std::thread th;
 
     void run()
@@ -56,7 +57,13 @@ struct Tracer {
             }
             tri_sample s;
             memset(&s, 0, sizeof(s));
-            nvml::read_sample(api, dev, &s);
+            // the energy counter is the one slow NVML query (4-13 ms): read it about every 100 ms and carry the value
+            // forward in between, so that the clock / temperature / power samples keep the requested period
+            const size_t every = period_us >= 100000 ? 1 : (100000 + period_us - 1) / period_us;
+            const bool with_energy = (i % every) == 0;
+            s.energy_mj = last_energy_mj;
+            nvml::read_sample(api, dev, &s, with_energy);
+            last_energy_mj = s.energy_mj;
             s.t_s = now_s() - t0;                      // stamped after the reads: the values are at most this old
             s.phase = phase.load(std::memory_order_acquire);
             buf[i] = s;
