@@ -345,3 +345,39 @@ def tri_fit_power(ai, f_mhz, p_w, eta, beta, f_sel_mhz, f_tol_mhz, p_cap_w):
     _check(lib().tri_fit_power((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*p_w), n, byref(m.c), f_sel_mhz, f_tol_mhz,
                                p_cap_w, byref(pi), byref(pd), byref(used)), "tri_fit_power")
     return {"p_idle_w": pi.value, "p_dyn_w": pd.value, "n_used": used.value}
+
+
+# the C names of the row-f3 entry points, on a Model
+def tri_model_theta(model: Model, ai: float, f_mhz: float) -> float:
+    return model.theta(ai, f_mhz)
+
+
+def tri_model_phi(model: Model, ai: float, f_mhz: float) -> float:
+    return model.phi(ai, f_mhz)
+
+
+def tri_model_power(model: Model, ai: float, i: int) -> float:
+    return model.power(ai, i)
+
+
+def tri_solve_clock(model: Model, ai: float, f_limit_mhz: float, eps: float):
+    return model.solve_clock(ai, f_limit_mhz, eps)
+
+
+# the remaining C names, as thin aliases of the wrappers above
+tri_status_string = status_string
+tri_last_error = last_error
+tri_sm_count = sm_count
+tri_l2_bytes = l2_bytes
+
+
+def phase_trace_start(device: int = 0, period_us: int = 10000, capacity: int = 65536, phase: int = TRI_PHASE_IDLE) -> PhaseTracer:
+    return PhaseTracer(device, period_us, capacity).start(phase)
+
+
+def phase_trace_mark(tracer: PhaseTracer, phase: int) -> None:
+    tracer.mark(phase)
+
+
+def phase_trace_stop(tracer: PhaseTracer) -> list:
+    return tracer.stop()

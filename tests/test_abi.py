@@ -117,3 +117,8 @@ def test_product_does_not_import_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(base, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text and "oracle/" not in text, f
+
+
+def test_binding_has_every_c_name():
+    """The Python binding mirrors the C ABI name for name (argument marshalling only)."""
+    assert [n for n in tri.EXPORTS if not hasattr(tri, n)] == []
