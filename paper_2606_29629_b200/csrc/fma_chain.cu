@@ -124,9 +124,10 @@ static int run(unsigned k, float a, float b, size_t n, const float *in, float *o
     }
     // float4 loads in flight per thread (= 4 x VEC chains), chosen by measurement on B200 (N = 2^28): the memory-bound
     // end likes many small blocks (VEC 2: 6.85 TB/s), the ridge needs both the load queue and the FP32 pipe full
-    // (VEC 4 at k = 32, VEC 8 from k = 48: 0.95-0.98 of the ALU roof instead of 0.90-0.96), the far compute-bound end
+    // (VEC 4 at k = 32, VEC 8 from k = 40: 1.04 of the HBM roof there instead of 0.96, 0.95-0.98 of the ALU roof from k = 48
+    // instead of 0.90-0.96; VEC 16 is no better), the far compute-bound end
     // is indifferent (VEC 2: 0.998).
-    int vec = variant ? variant : (k <= 24 ? 2 : k <= 40 ? 4 : k < 2048 ? 8 : 2);
+    int vec = variant ? variant : (k <= 24 ? 2 : k <= 35 ? 4 : k < 2048 ? 8 : 2);
     cudaError_t e;
     switch (vec) {
         case 1: e = launch<1>(in, out, n, k, a, b, s); break;
