@@ -191,9 +191,9 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
     auto stage = [&](auto cur_tag, int s) {
         constexpr int CUR = decltype(cur_tag)::value, NXT = CUR ^ 1;
         const uint32_t base = ring + slot * GV_SLOT_BYTES;
-        uint32_t xv[MR][KN ? 2 : 4];
+        [[maybe_unused]] uint32_t xv[MR][KN ? 2 : 4];
         constexpr bool XT = GV_XT_ENABLED && MR == 8;                 // X transposed to row pairs per k (see below)
-        uint32_t xq[XT ? 8 : 1][4];
+        [[maybe_unused]] uint32_t xq[XT ? 8 : 1][4];
         if constexpr (XT && !KN) {
             // lane (kp, rq) of the half-warp: rows 2rq, 2rq+1 at k-pair kp of the chunk -> words (row pair at k), (row pair at k+1)
             const int kp = i16 >> 2, rq = i16 & 3;
