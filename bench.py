@@ -6,8 +6,11 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
-Prints ONE JSON line (see DESIGN.md "Measurement").  `value` is the aggregate algorithmic TFLOP/s of the step;
-the per-A.I.-point GB/s, TFLOP/s and % of roofline (the metric BASELINE.json names) are in `points`.
+stdout carries exactly ONE compact JSON line (< 3 KB): `value` is the aggregate
+algorithmic TFLOP/s of the step (fp32-FMA and bf16-tensor FLOP blended by the workload's own mix), `fracs` / `min_frac`
+are the fractions of roofline per A.I. point — the metric BASELINE.json names — and `roofline`, `cpu_baseline`, `e2e`
+the objects of the bench contract.  The full per-point detail (GB/s, TFLOP/s, clock, temperature, power, J/op, model
+fit) goes to gpurun_out/bench_points.json and, one JSON line per point, to stderr.
 `--impl reference` times the CPU oracle, as it stands, on a bounded sample of the same step.
 """
 from __future__ import annotations
@@ -109,8 +112,7 @@ class OracleSample:
         self.ga = normal_bf16(3, (self.GEMM_ROWS, k), 1.0, stream=0)
         self.flop = (sum(fma_flop(kk, self.N_FMA_S) for kk in KS) + gemm_flop(GEMV_SHAPE)
                      + gemm_flop((self.GEMM_ROWS, n, k)))
-        self.desc = (f"per step: FMA chain 2^18 of 2^28 elements at each of 13 k; config-3 GEMV once (of 8); "
-                     f"{self.GEMM_ROWS} of 4096 rows of the config-4 GEMM")
+        self.desc = f"per step: 2^18 of 2^28 elements per k (13 k); 1 of 8 GEMVs; {self.GEMM_ROWS} of 4096 GEMM rows"
 
     def step(self):
         t0 = time.perf_counter()
@@ -132,12 +134,12 @@ def run_reference(args):
     tot = sum(times)
     value = s.flop * args.steps / tot / 1e12
     cores = s.oracle.num_threads()
-    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": "TFLOP/s (algorithmic, whole step)",
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
            "data": "synthetic", "config": workload_config(args.gpus),
            "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "sample": s.desc},
-           "e2e": {"value": value, "unit": "TFLOP/s (algorithmic, whole step)", "h2d_bytes_per_step": 0,
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
                    "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out), flush=True)
@@ -145,9 +147,9 @@ def run_reference(args):
 
 def workload_config(n_gpus):
     return {"workload": "configs[1] A.I. sweep (FMA chain N=2^28 fp32, k=2^0..2^12) + configs[2] decode GEMV 8x3584x18944 "
-                        "x 8 rotating weight copies + configs[3] prefill GEMM 4096x3584x18944, W layout NK",
+                        "x 8 rotating W copies + configs[3] prefill GEMM 4096x3584x18944; W layout NK",
             "parallelism": f"replicas x{n_gpus} (no collective)",
-            "l2": "inputs larger than L2 (2 GiB FMA stream; 8 rotating 136 MB GEMV weights; 320 MB GEMM operands)"}
+            "l2": "inputs larger than L2 (2 GiB stream; 8 x 136 MB GEMV weights; 320 MB GEMM operands)"}
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -227,7 +229,7 @@ def summarise_clocks(samples, peaks):
     reasons = [name for bit, name in REASONS.items() if bits & bit and name != "gpu_idle"]
     return {"sm_mhz": statistics.median(s["sm_mhz"] for s in busy), "sm_max_mhz": peaks["sm_max_mhz"],
             "reasons": reasons, "temp_c_max": max(s["temp_c"] for s in busy),
-            "power_w_mean": sum(s["power_w"] for s in busy) / len(busy), "samples": len(busy), "source": "nvml via phase_trace_start"}
+            "power_w_mean": sum(s["power_w"] for s in busy) / len(busy), "samples": len(busy), "source": "nvml"}
 
 
 def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
@@ -328,6 +330,70 @@ def gemm_ai_series(torch, tri, peaks):
                     "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9})
         del a, w, c
     return out
+
+
+UNIT = "TFLOP/s (algorithmic, whole step: fp32-FMA + bf16-tensor FLOP)"
+DETAIL_FILE = os.path.join("gpurun_out", "bench_points.json")
+COMPACT_KEYS = ["impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "min_frac"]
+
+
+def point_key(pt):
+    if pt["kernel"] == "fma_chain":
+        return f"fma_k{pt['k']}"
+    return {"decode_gemv": "gemv", "prefill_gemm": "gemm"}[pt["kernel"]]
+
+
+def sig(x, digits=4):
+    return None if x is None else float(f"{x:.{digits}g}")
+
+
+def compact_line(full):
+    """The ONE line of stdout: the bench contract's keys, plus the metric BASELINE.json names in compact form —
+    `fracs` = fraction of roofline per A.I. point (burst, per-launch CUDA-event medians of the timed steps) and
+    `sustained` = per point [fraction of the roofline at the recorded clock, SM MHz, W, pJ/FLOP] from the looped pass
+    (the ridge and paper-A.I. extra series are in the detail file only).
+    Everything bulky (`points`, `extra_points`, `model_fit`) stays in the detail file.  Kept under 3 KB: the round-1
+    line was 20 KB and the driver could not parse it."""
+    out = {k: full[k] for k in COMPACT_KEYS if k in full}
+    pts = full.get("points") or []
+    out["fracs"] = {point_key(p): round(p["frac"], 3) for p in pts}
+    sus = {}
+    for p in pts:
+        c = p.get("sustained")
+        if c and p.get("frac_sustained_at_clock") is not None:
+            pj = c.get("j_per_flop")
+            sus[point_key(p)] = [round(p["frac_sustained_at_clock"], 3), int(c.get("sm_mhz") or 0), int(c.get("power_w_mean") or 0),
+                                 sig(pj * 1e12 if pj else None, 3)]
+    if sus:
+        out["sustained"] = sus
+        out["sustained_cols"] = "frac at recorded clock, SM MHz, W, pJ/FLOP"
+    gm = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "prefill_gemm" and q.get("label")]
+    if gm:
+        out["gemm_shapes"] = {q["label"]: round(q["frac"], 3) for q in gm}
+    if full.get("energy"):
+        out["j_per_flop"] = sig(full["energy"].get("j_per_flop"), 3)
+    out["detail"] = DETAIL_FILE
+    for k in ("value", "ms_per_step", "min_frac"):
+        if isinstance(out.get(k), float):
+            out[k] = sig(out[k], 6)
+    return json.dumps(out, separators=(",", ":"))
+
+
+def emit(full):
+    """Detail first (file + one JSON line per point on stderr), then the single compact line on stdout."""
+    try:
+        os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+        with open(os.path.join(ROOT, DETAIL_FILE), "w") as f:
+            json.dump(full, f, indent=1)
+    except OSError as e:
+        print(f"bench.py: could not write {DETAIL_FILE}: {e}", file=sys.stderr)
+    for p in (full.get("points") or []) + (full.get("extra_points") or []):
+        print(json.dumps(p), file=sys.stderr)
+    if full.get("model_fit"):
+        print(json.dumps({"model_fit": full["model_fit"]}), file=sys.stderr)
+    sys.stderr.flush()
+    print(compact_line(full), flush=True)
 
 
 def run_ours(args):
@@ -476,26 +542,27 @@ def run_ours(args):
     traffic = ncu_traffic_bytes("fma_chain", column=len(KS) - 1)
     roofline = {"kernel": "fma_chain_kernel (k=4096 launch)", "bound": "alu", "achieved": dom["tflops"], "peak": alu_peak,
                 "unit": "TFLOP/s", "frac": dom["tflops"] / alu_peak, "traffic": traffic,
-                "peak_source": f"derived: {sms} SMs x {FP32_LANES_PER_SM} fp32 FMA lanes x 2 FLOP x {peaks['sm_max_mhz']:.0f} MHz "
-                               f"(max SM clock, {peaks['source']}); hbm / tensor points in `points` use MEASURED_PEAKS.json "
-                               f"({peaks['source']}): {peaks['hbm_gbs']} GB/s, {peaks['bf16_tflops']} TFLOP/s burst"}
+                "share_of_step": dom["ms"] * args.steps / total_ms,
+                "peak_source": f"derived {sms} SMs x {FP32_LANES_PER_SM} lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz; fracs: {peaks['source']} "
+                               f"{peaks['hbm_gbs']} GB/s, {peaks['bf16_tflops']} TFLOP/s"}
 
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----
     e2e = run_e2e(torch, tri, step, args, barrier, dist)
 
     value = whole_job_value(STEP_FLOP, args.steps, world, total_ms)
     energy_j = (e1 - e0) * 1e-3 if e1 > e0 else None
-    out = {"metric": METRIC, "value": value, "unit": "TFLOP/s (algorithmic, whole step)", "n_gpus": world,
-           "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
-           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
-           "data": "synthetic", "config": workload_config(world), "clocks": dict(clocks, sm_mhz_in_kernel_probe=clk_probe),
-           "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points, "extra_points": extra_points, "model_fit": model_fit,
-           "min_frac": min(p["frac"] for p in points),
-           "energy": {"j_per_step": energy_j / args.steps if energy_j else None,
-                      "j_per_flop": energy_j / (STEP_FLOP * args.steps) if energy_j else None,
-                      "j_per_byte": energy_j / (STEP_BYTES * args.steps) if energy_j else None},
-           "paper_context": "Tri-serve reports -22.1 % J/output-token on 3x RTX 6000 Ada (Qwen2.5-Omni-7B, vLLM-Omni); "
-                            "no throughput number is published for this path (BASELINE.md)"}
+    full = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 chain; bf16 in / f32 acc",
+            "data": "synthetic", "config": workload_config(world), "clocks": dict(clocks, sm_mhz_in_kernel_probe=clk_probe),
+            "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points,
+            "extra_points": extra_points, "model_fit": model_fit, "min_frac": min(p["frac"] for p in points),
+            "energy": {"j_per_step": energy_j / args.steps if energy_j else None,
+                       "j_per_flop": energy_j / (STEP_FLOP * args.steps) if energy_j else None,
+                       "j_per_byte": energy_j / (STEP_BYTES * args.steps) if energy_j else None},
+            "peaks": peaks,
+            "paper_context": "Tri-serve reports -22.1 % J/output-token on 3x RTX 6000 Ada (Qwen2.5-Omni-7B, vLLM-Omni); "
+                             "no throughput number is published for this path (BASELINE.md)"}
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             s = OracleSample()
@@ -504,9 +571,9 @@ def run_ours(args):
             while t < 10.0 and reps < 50:
                 t += s.step()
                 reps += 1
-            out["cpu_baseline"] = {"value": s.flop * reps / t / 1e12, "unit": "TFLOP/s", "cores": s.oracle.num_threads(),
-                                   "kind": "oracle", "sample": s.desc + f"; {reps} repetitions, {t:.1f} s"}
-        print(json.dumps(out), flush=True)
+            full["cpu_baseline"] = {"value": s.flop * reps / t / 1e12, "unit": "TFLOP/s", "cores": s.oracle.num_threads(),
+                                    "kind": "oracle", "sample": s.desc + f"; {reps} repetitions, {t:.1f} s"}
+        emit(full)
     if dist is not None:
         dist.destroy_process_group()
 
@@ -576,9 +643,9 @@ def run_e2e(torch, tri, step, args, barrier, dist):
     ok = bool(torch.equal(hy[:4096], ref[:4096].cpu()))                # the read-back is the last step's result
     ms = max_over_ranks(ms, dist, "cuda")
     world = dist.get_world_size() if dist is not None else 1
-    return {"value": whole_job_value(STEP_FLOP, n, world, ms), "unit": "TFLOP/s (algorithmic, whole step)",
+    return {"value": whole_job_value(STEP_FLOP, n, world, ms), "unit": UNIT,
             "ms_per_step": ms / n, "steps": n, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-            "overlap": "3 streams, 2 buffer sets: H2D(i+1) | kernels(i) | D2H(i-1)", "readback_checked": ok}
+            "overlap": "H2D(i+1) | kernels(i) | D2H(i-1)", "readback_checked": ok}
 
 
 def main():
