@@ -103,6 +103,52 @@ int make_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64
     return TRI_OK;
 }
 
+// Direct-mapped cache of encoded maps.  cuTensorMapEncodeTiled costs about a microsecond per map, a 20 us decode_gemv
+// needs two and a prefill_gemm three; serving loops call with the same buffers every step.
+struct TmapKey {
+    const void *base;
+    uint64_t inner, outer, pitch;
+    uint32_t box_inner, box_outer;
+    int swz;
+    bool operator==(const TmapKey &o) const
+    {
+        return base == o.base && inner == o.inner && outer == o.outer && pitch == o.pitch && box_inner == o.box_inner &&
+               box_outer == o.box_outer && swz == o.swz;
+    }
+};
+struct TmapEntry {
+    bool valid = false;
+    TmapKey key;
+    CUtensorMap map;
+};
+constexpr int TMAP_CACHE_SIZE = 256;
+static TmapEntry g_tmaps[TMAP_CACHE_SIZE];
+static std::mutex g_tmap_mu;
+
+int cached_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer, uint64_t pitch_bytes,
+                        uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz)
+{
+    const TmapKey key{base, inner, outer, pitch_bytes, box_inner, box_outer, (int)swz};
+    uint64_t h = (uint64_t)(uintptr_t)base * 0x9E3779B97F4A7C15ull;
+    h ^= (inner * 0xBF58476D1CE4E5B9ull) ^ (outer * 0x94D049BB133111EBull) ^ (pitch_bytes << 17) ^ ((uint64_t)box_inner << 40) ^
+         ((uint64_t)box_outer << 48) ^ ((uint64_t)swz << 56);
+    TmapEntry &e = g_tmaps[(h ^ (h >> 29)) % TMAP_CACHE_SIZE];
+    {
+        std::lock_guard<std::mutex> lk(g_tmap_mu);
+        if (e.valid && e.key == key) {
+            *map = e.map;
+            return TRI_OK;
+        }
+    }
+    int st = make_tmap_2d_bf16(map, base, inner, outer, pitch_bytes, box_inner, box_outer, swz);
+    if (st != TRI_OK) return st;
+    std::lock_guard<std::mutex> lk(g_tmap_mu);
+    e.key = key;
+    e.map = *map;
+    e.valid = true;
+    return TRI_OK;
+}
+
 // One block, one thread: spins until `spin_ns` of %globaltimer have passed and reports both clocks.
 __global__ void sm_clock_probe(unsigned long long spin_ns, unsigned long long *out)
 {

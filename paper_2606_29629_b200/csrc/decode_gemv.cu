@@ -1,73 +1,61 @@
 // a2. Decode-phase GEMV ("GEMV-like operators"; BASELINE.json config 3; ABI in
 // include/triroof.h):   Y[m][n] = bf16_rne( sum_k X[m][k] * W[k][n] ),  m <= 16, fp32 accumulation.
 //
-// HBM-bound: the weight matrix is read exactly once.  CUDA-core kernel by design (the GEMM is the
-// only tensor-core path).  The arithmetic is the sm_100 mixed-precision FMA  fma.rn.f32.bf16
-// (SASS FHFMA.BF16): d = a * b + c with a, b bf16 taken from either half of a 32-bit register and c, d
-// fp32, one rounding — bit-identical to fmaf on the widened inputs, at the full FP32 rate (measured:
-// 125 of 128 lanes/clk/SM) and with no unpack instruction at all.  So the packed bf16 words of W and X
-// go from shared memory straight into the FMA, and a weight costs m FMA-pipe slots.
+// HBM-bound: the weight matrix is read exactly once, whatever m is.  One skeleton, both layouts: a CTA owns 64 output
+// columns; 4 compute warps + 1 producer warp (160 threads), TWO CTAs per SM (18944 = 296 * 64: one wave on 148 SMs),
+// so the prologue and the tail of one CTA are covered by its neighbour and, with programmatic dependent launch, by
+// the first CTAs of the next call.
+//   * producer warp (one lane): per 64-k stage one TMA box of W (64 x 64 bf16 = 8 KiB, 128-byte swizzle, L2
+//     evict-first) and one of X (64 k x 8 or 16 rows; rows >= m and k >= K arrive as zeros) into a ring of ten
+//     slots; full / empty mbarriers.  X rides in the ring, so there is no prologue, no limit on K, and nothing but
+//     the ring in shared memory.
 //
-// What limits it (measured, B200): the register file has two banks (even / odd register numbers) and each delivers
-// one new register per cycle; an operand held over from the previous instruction (.reuse) is free.  A scalar FMA
-// with three distinct operands therefore issues every 2 cycles unless one operand is reused, and ptxas interleaves
-// the FMA stream so that about half of them miss (1.5 cycles per FMA; forcing the order through data or control
-// dependencies cost as much in bubbles).  For m <= 4 the kernel stays HBM-bound (21.7 us at m = 1, 22.8 us at m = 4 on
-// the config-3 shape with the 8-slot ring; 20.1 / 21.2 us = 103 % / 98 % of the measured copy peak with 10 slots); at m = 5..8 it is
-// FMA-issue bound (39 us NK, 29 us KN as first written; 28.3 / 27.8 us with X transposed to row pairs, see below),
-// so TRI_W_NK with 5..8 rows and k <= 4096 goes to the packed-FFMA2 kernel of decode_gemv_m8.cu (24.8 us), whose
-// 64-bit operands read one register of each bank and cannot conflict.
+// Two arithmetic paths behind it:
 //
-// One kernel, both layouts.  A CTA owns 64 output columns; 4 compute warps + 1 producer warp (160
-// threads), TWO CTAs per SM (18944 = 296 * 64: one wave on 148 SMs), so the prologue, the reduction
-// and the tail of one CTA are covered by its neighbour and, with programmatic dependent launch, by the
-// first CTAs of the next call.
-//   * producer warp (one lane): per 64-k stage one TMA box of W (64 x 64 bf16 = 8 KiB, 128-byte
-//     swizzle, L2 evict-first) and one of X (64 k x 8 rows = 1 KiB; rows >= m and k >= K arrive as
-//     zeros) into a ring of 9 KiB slots; full / empty mbarriers.  X rides in the ring, so there is no
-//     prologue, no limit on K, and nothing but the ring in shared memory.
-//   * compute warps, TRI_W_NK (slot row = column n, 128 B = 64 k): half-warp h of warp w owns the
-//     8-k chunk 2w + h of the stage, lane i of it the columns i, i+16, i+32, i+48: four LDS.128 of
-//     W (the swizzle puts the 8 lanes of a quarter-warp on 8 different 16-byte bank groups), eight
-//     broadcast LDS.128 of X (row mm, same chunk), 4 x 8 x 8 = 256 FMAs.
-//   * compute warps, TRI_W_KN (slot row = k, 128 B = 64 columns n): lane (c = lane & 7, q = lane >> 3)
-//     of warp w owns the 8 columns of chunk c and the k-rows 16w + 4q .. + 3: four LDS.128 of W (a
-//     quarter-warp reads one whole row), eight broadcast LDS.64 of X, 8 x 4 x 8 = 256 FMAs.
-//   * 8-row kernels: each (half-)warp first transposes its slice of X to row PAIRS per k (2 LDS.32, 2 PRMT, 2 STS.32 per
-//     lane and stage), so that one X word holds rows (2q, 2q+1) at one k.  Two (NK) or four (KN) independent FMAs then
-//     use the same two registers, which is the operand pattern that needs no register-file read (tri_probe_fma_issue
-//     pattern 0) and the one ptxas keeps together; statically 1.17 instead of 1.4-1.6 issue cycles per FMA;
-//   * the W registers of stage s + 1 are loaded before the FMAs of stage s, and a slot is released as
-//     soon as its words are in registers.
-//   * after the last stage the partial sums (8 sets for NK, 16 for KN) are added through shared
-//     memory (the ring is dead by then), rounded to bf16 RNE and stored.
+// (1) m <= 4: CUDA cores, the sm_100 mixed-precision FMA  fma.rn.f32.bf16  (SASS FHFMA.BF16): d = a * b + c with a, b
+//     bf16 taken from either half of a 32-bit register and c, d fp32, one rounding — bit-identical to fmaf on the
+//     widened inputs, at the full FP32 rate and with no unpack instruction.  A weight costs m FMA-pipe slots;
+//     measured on the config-3 shape: 20.1 us at m = 1, 21.2 us at m = 4 (103 % / 98 % of the measured copy peak).
+//       - TRI_W_NK (slot row = column n, 128 B = 64 k): half-warp h of warp w owns the 8-k chunk 2w + h of the stage,
+//         lane i of it the columns i, i+16, i+32, i+48: four LDS.128 of W, m broadcast LDS.128 of X, 4 x 8 x m FMAs;
+//         8 partial sums per output are added through shared memory at the end.
+//       - TRI_W_KN (slot row = k, 128 B = 64 columns n): lane (c = lane & 7, q = lane >> 3) of warp w owns the 8
+//         columns of chunk c and the k-rows 16w + 4q .. + 3; 16 partial sums per output.
+//
+// (2) 5 <= m <= 16: the warp-level tensor-core instruction  mma.sync.m16n8k16 (bf16 in, fp32 accumulate; SASS HMMA)
+//     with the WEIGHT tile as the 16-row operand and the batch as n = 8 (one tile for m <= 8, two for m <= 16): zero
+//     padding waste at m = 8, and W is still read once at m = 16.  Why not CUDA cores here (DESIGN.md §5.2 has the
+//     numbers): m FMAs per weight are 14.6 us of FMA-pipe time at m = 8 and 1965 MHz (17 us at the ~1.7 GHz the part
+//     holds under its power cap) inside a 20.8 us HBM budget, and 29 us at m = 16 — the round-1 FFMA2 / FHFMA kernels
+//     stopped at 24.8 us back to back and 26.9 us inside the bench step (0.77 of the roofline) with the FMA pipe 60 %
+//     busy and no other unit saturated.  SURVEY.md §7.3-B names this instruction as the escape hatch; the stream, the
+//     ring and the accounting are unchanged, only the inner product moved.  Warp w owns the 16 columns 16w .. 16w+15
+//     of the CTA over ALL k (no cross-warp reduction): per 64-k stage four ldmatrix.x4 of W (conflict-free on the
+//     128-byte swizzle; .trans for TRI_W_KN), two ldmatrix.x4 of X per batch tile, four mma per batch tile, alternating
+//     between two accumulator sets.
 #include "tri_internal.h"
 #include "ptx.cuh"
 
 #include <cuda_bf16.h>
-#include <cstdlib>
 
 namespace tri {
 
-constexpr int GV_M = 8;                  // batch rows per launch (the X box is always 8 rows; missing rows are zeros)
 constexpr int GV_COLS = 64;              // output columns per CTA
 constexpr int GV_CWARPS = 4;             // compute warps
 constexpr int GV_CTHREADS = GV_CWARPS * 32;
 constexpr int GV_THREADS = GV_CTHREADS + 32;          // + producer warp
 constexpr int GV_STAGE_K = 64;           // k-values per stage
 constexpr int GV_W_BYTES = GV_STAGE_K * GV_COLS * 2;  // 8 KiB
-constexpr int GV_X_BYTES = GV_STAGE_K * GV_M * 2;     // 1 KiB
-constexpr int GV_SLOT_BYTES = GV_W_BYTES + GV_X_BYTES;
-constexpr int GV_MAX_SLOTS = 12;
-#ifndef GV_XT_ENABLED
-#define GV_XT_ENABLED 1      // 8-row kernels read X transposed to row pairs (0: A/B comparison only)
-#endif
-constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS + 8 * 128;   // full[], empty[], per-half-warp transposition scratch
-constexpr int GV_RED_STRIDE = GV_M * GV_COLS + 16;    // floats per partial-sum set; +16 keeps the two half-warps on different banks
+constexpr int GV_XROW_BYTES = GV_STAGE_K * 2;         // 128 B: one batch row of a stage
+constexpr int GV_MAX_SLOTS = 10;
+constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS;    // full[], empty[]
+constexpr int GV_RED_STRIDE = 4 * GV_COLS + 16;       // FHFMA path: floats per partial-sum set; +16 keeps the two half-warps on different banks
 
-__host__ __device__ constexpr size_t gemv_smem_bytes(int nslots)
+// X rows per slot: 8 for the FHFMA path and one batch tile of the MMA path, 16 for two tiles.
+__host__ __device__ constexpr int gemv_slot_bytes(int xrows) { return GV_W_BYTES + xrows * GV_XROW_BYTES; }
+__host__ __device__ constexpr size_t gemv_smem_bytes(int nslots, int xrows)
 {
-    return 1024 + (size_t)nslots * GV_SLOT_BYTES + GV_BAR_BYTES;
+    return 1024 + (size_t)nslots * gemv_slot_bytes(xrows) + GV_BAR_BYTES;
 }
 
 // acc + w.half * x.half: the sm_100 mixed-precision FMA (SASS FHFMA.BF16; the half selects become operand modifiers of
@@ -94,66 +82,108 @@ __device__ __forceinline__ void lds64(uint32_t (&r)[2], uint32_t addr)
 {
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(addr));
 }
+// Four 8 x 8 bf16 matrices, row addresses from lanes 8j .. 8j+7; thread (g = lane / 4, t = lane % 4) gets elements
+// (g, 2t), (g, 2t+1) of matrix j in r[j] — (2t, g), (2t+1, g) with TRANS.
+template <bool TRANS>
+__device__ __forceinline__ void ldmatrix_x4(uint32_t (&r)[4], uint32_t addr)
+{
+    if constexpr (TRANS)
+        asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+    else
+        asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(addr));
+}
+// D (16 x 8, fp32) += A (16 x 16, row) * B (16 x 8, col), bf16 inputs: the warp-level tensor-core MMA.
+__device__ __forceinline__ void mma_16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%0, %1, %2, %3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
 
-// MR: batch rows computed (1, 2, 4 or 8 >= m).  KN: W_phys[k][n] (slot row = k) instead of W_phys[n][k] (slot row = n).
+struct GemvBars {
+    uint32_t ring, full0, empty0;
+};
+
+// Carves the dynamic shared memory (1 KiB aligned: 128-byte swizzle atoms), initialises the barriers and lets the next
+// kernel of the stream start its CTAs as SM resources free up (programmatic dependent launch).
+template <int SLOT_BYTES>
+__device__ __forceinline__ GemvBars gemv_setup(uint8_t *smem_raw, int nslots, uint8_t **aligned)
+{
+    const uint32_t base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    *aligned = smem_raw + (base - ptx::smem_u32(smem_raw));
+    GemvBars b;
+    b.ring = base;
+    b.full0 = base + nslots * SLOT_BYTES;
+    b.empty0 = b.full0 + 8 * GV_MAX_SLOTS;
+    ptx::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < nslots; ++s) {
+            ptx::mbar_init(b.full0 + 8 * s, 1);
+            ptx::mbar_init(b.empty0 + 8 * s, GV_CWARPS);
+        }
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();
+    return b;
+}
+
+// Producer (one lane): streams the CTA's weight panel and the matching X slices through the ring.  W (model state,
+// never an output of the preceding kernel) is fetched at once; X is fetched only after pdl_wait(), i.e. after the
+// preceding grid has completed (aliasing rule in include/triroof.h).
+template <int SLOT_BYTES, bool KN>
+__device__ __forceinline__ void gemv_producer(const GemvBars &b, const CUtensorMap *wmap, const CUtensorMap *xmap, int n0,
+                                              int nstages, int nslots)
+{
+    ptx::prefetch_tmap(wmap);
+    ptx::prefetch_tmap(xmap);
+    const uint64_t pol_w = ptx::policy_evict_first();          // weights are read once
+    const uint64_t pol_x = ptx::policy_evict_last();           // X is re-read by every CTA
+    const int npre = nstages < nslots ? nstages : nslots;
+    for (int s = 0; s < npre; ++s) {
+        const uint32_t fb = b.full0 + 8 * s;
+        ptx::mbar_arrive_expect_tx(fb, SLOT_BYTES);
+        if (KN) ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, n0, s * GV_STAGE_K, fb, pol_w);
+        else ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, s * GV_STAGE_K, n0, fb, pol_w);
+    }
+    ptx::pdl_wait();
+    for (int s = 0; s < npre; ++s)
+        ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES + GV_W_BYTES, xmap, s * GV_STAGE_K, 0, b.full0 + 8 * s, pol_x);
+    int slot = 0;
+    uint32_t par = 0;                                          // parity of the slot's first release
+    for (int s = npre; s < nstages; ++s) {
+        ptx::mbar_wait(b.empty0 + 8 * slot, par);
+        const uint32_t fb = b.full0 + 8 * slot, dst = b.ring + slot * SLOT_BYTES;
+        ptx::mbar_arrive_expect_tx(fb, SLOT_BYTES);
+        if (KN) ptx::tma_load_2d_hint(dst, wmap, n0, s * GV_STAGE_K, fb, pol_w);
+        else ptx::tma_load_2d_hint(dst, wmap, s * GV_STAGE_K, n0, fb, pol_w);
+        ptx::tma_load_2d_hint(dst + GV_W_BYTES, xmap, s * GV_STAGE_K, 0, fb, pol_x);
+        if (++slot == nslots) { slot = 0; par ^= 1; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// (1) CUDA-core path.  MR: batch rows computed (1, 2 or 4 >= m).  KN: W_phys[k][n] (slot row = k) instead of W_phys[n][k].
+// ---------------------------------------------------------------------------------------------------------------------
 template <int MR, bool KN>
 __global__ void __launch_bounds__(GV_THREADS, 2)
 gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap xmap, uint16_t *__restrict__ y,
             int64_t ldy, int m, int n, int k, int nslots)
 {
+    constexpr int SLOT = gemv_slot_bytes(8);
     extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;     // 128-byte swizzle atoms are 1 KiB
-    float *red = reinterpret_cast<float *>(smem_raw + (smem_base - ptx::smem_u32(smem_raw)));
-    const uint32_t ring = smem_base;
-    const uint32_t full0 = smem_base + nslots * GV_SLOT_BYTES;
-    const uint32_t empty0 = full0 + 8 * GV_MAX_SLOTS;
+    uint8_t *smem;
+    const GemvBars b = gemv_setup<SLOT>(smem_raw, nslots, &smem);
+    float *red = reinterpret_cast<float *>(smem);
+    const uint32_t ring = b.ring, full0 = b.full0, empty0 = b.empty0;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int n0 = blockIdx.x * GV_COLS;
     const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
 
-    // Programmatic dependent launch: the next kernel of the stream may start its CTAs as SM resources free up.
-    // W (model state, never an output of the preceding kernel) is fetched at once; X is fetched and Y is written
-    // only after pdl_wait(), i.e. after the preceding grid has completed (aliasing rule in include/triroof.h).
-    ptx::pdl_launch_dependents();
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < nslots; ++s) {
-            ptx::mbar_init(full0 + 8 * s, 1);
-            ptx::mbar_init(empty0 + 8 * s, GV_CWARPS);
-        }
-        ptx::fence_mbar_init();
-    }
-    __syncthreads();
-
     if (warp == GV_CWARPS) {
-        // ===== producer warp: one lane streams the CTA's weight panel and the matching X slices =====
-        if (lane == 0) {
-            ptx::prefetch_tmap(&wmap);
-            ptx::prefetch_tmap(&xmap);
-            const uint64_t pol_w = ptx::policy_evict_first();          // weights are read once
-            const uint64_t pol_x = ptx::policy_evict_last();           // X is re-read by every CTA
-            const int npre = nstages < nslots ? nstages : nslots;
-            for (int s = 0; s < npre; ++s) {
-                const uint32_t fb = full0 + 8 * s;
-                ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
-                if (KN) ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES, &wmap, n0, s * GV_STAGE_K, fb, pol_w);
-                else ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES, &wmap, s * GV_STAGE_K, n0, fb, pol_w);
-            }
-            ptx::pdl_wait();
-            for (int s = 0; s < npre; ++s)
-                ptx::tma_load_2d_hint(ring + s * GV_SLOT_BYTES + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, full0 + 8 * s, pol_x);
-            int slot = 0;
-            uint32_t par = 0;                                          // parity of the slot's first release
-            for (int s = npre; s < nstages; ++s) {
-                ptx::mbar_wait(empty0 + 8 * slot, par);
-                const uint32_t fb = full0 + 8 * slot, dst = ring + slot * GV_SLOT_BYTES;
-                ptx::mbar_arrive_expect_tx(fb, GV_SLOT_BYTES);
-                if (KN) ptx::tma_load_2d_hint(dst, &wmap, n0, s * GV_STAGE_K, fb, pol_w);
-                else ptx::tma_load_2d_hint(dst, &wmap, s * GV_STAGE_K, n0, fb, pol_w);
-                ptx::tma_load_2d_hint(dst + GV_W_BYTES, &xmap, s * GV_STAGE_K, 0, fb, pol_x);
-                if (++slot == nslots) { slot = 0; par ^= 1; }
-            }
-        }
+        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, nstages, nslots);
         return;
     }
 
@@ -179,8 +209,6 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
         xoff = GV_W_BYTES + (uint32_t)chunk * 16u;
     }
 
-    const uint32_t xt_scratch = empty0 + 8 * GV_MAX_SLOTS + (uint32_t)(warp * 2 + (lane >> 4)) * 128u;   // per half-warp, 8 k x 16 B
-    const uint32_t xt_warp = empty0 + 8 * GV_MAX_SLOTS + (uint32_t)warp * 256u;                       // KN: per warp, 16 k x 16 B
     uint32_t wv[2][4][4];
     int slot = 0;
     uint32_t par = 0;
@@ -190,64 +218,23 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
 
     auto stage = [&](auto cur_tag, int s) {
         constexpr int CUR = decltype(cur_tag)::value, NXT = CUR ^ 1;
-        const uint32_t base = ring + slot * GV_SLOT_BYTES;
-        [[maybe_unused]] uint32_t xv[MR][KN ? 2 : 4];
-        constexpr bool XT = GV_XT_ENABLED && MR == 8;                 // X transposed to row pairs per k (see below)
-        [[maybe_unused]] uint32_t xq[XT ? 8 : 1][4];
-        if constexpr (XT && !KN) {
-            // lane (kp, rq) of the half-warp: rows 2rq, 2rq+1 at k-pair kp of the chunk -> words (row pair at k), (row pair at k+1)
-            const int kp = i16 >> 2, rq = i16 & 3;
-            uint32_t a, b;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base + xoff + (2 * rq) * 128 + kp * 4));
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(base + xoff + (2 * rq + 1) * 128 + kp * 4));
-            const uint32_t sc = xt_scratch + (uint32_t)(2 * kp) * 16u + (uint32_t)rq * 4u;
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sc), "r"(__byte_perm(a, b, 0x5410)) : "memory");
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sc + 16), "r"(__byte_perm(a, b, 0x7632)) : "memory");
-            __syncwarp();
+        const uint32_t base = ring + slot * SLOT;
+        uint32_t xv[MR][KN ? 2 : 4];
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) lds128(xq[kk], xt_scratch + kk * 16);
-        } else if constexpr (XT && KN) {
-            // the warp's 16 k-rows: lane (kp = lane >> 2, rq = lane & 3) transposes rows 2rq, 2rq+1 at k-pair kp; then every
-            // lane reads the row-pair words of its own 4 k-rows
-            const int kp = lane >> 2, rq = lane & 3;
-            uint32_t a, b;
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(base + GV_W_BYTES + (2 * rq) * 128 + (16 * warp + 2 * kp) * 2));
-            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b) : "r"(base + GV_W_BYTES + (2 * rq + 1) * 128 + (16 * warp + 2 * kp) * 2));
-            const uint32_t sw = xt_warp + (uint32_t)(2 * kp) * 16u + (uint32_t)rq * 4u;
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sw), "r"(__byte_perm(a, b, 0x5410)) : "memory");
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(sw + 16), "r"(__byte_perm(a, b, 0x7632)) : "memory");
-            __syncwarp();
-#pragma unroll
-            for (int t = 0; t < 4; ++t) lds128(xq[t], xt_warp + (uint32_t)(4 * q4 + t) * 16u);
-        } else {
-#pragma unroll
-            for (int mm = 0; mm < MR; ++mm) {
-                if constexpr (KN) lds64(xv[mm], base + xoff + mm * 128);
-                else lds128(xv[mm], base + xoff + mm * 128);
-            }
+        for (int mm = 0; mm < MR; ++mm) {
+            if constexpr (KN) lds64(xv[mm], base + xoff + mm * 128);
+            else lds128(xv[mm], base + xoff + mm * 128);
         }
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(empty0 + 8 * slot);          // this stage's words are in registers: free the slot
         if (++slot == nslots) { slot = 0; par ^= 1; }
         if (s + 1 < nstages) {
             ptx::mbar_wait(full0 + 8 * slot, par);
-            const uint32_t nb = ring + slot * GV_SLOT_BYTES;
+            const uint32_t nb = ring + slot * SLOT;
 #pragma unroll
             for (int j = 0; j < 4; ++j) lds128(wv[NXT][j], nb + woff[j]);
         }
-        if constexpr (KN && XT) {
-#pragma unroll
-            for (int t = 0; t < 4; ++t)                               // k-row of the lane
-#pragma unroll
-                for (int u = 0; u < 4; ++u)                           // word u = columns 2u, 2u + 1 of the chunk
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) {                     // rows 2q, 2q + 1: four FMAs on the same two words
-                        acc[2 * u][2 * q] = fma_bf16<0, 0>(wv[CUR][t][u], xq[t][q], acc[2 * u][2 * q]);
-                        acc[2 * u][2 * q + 1] = fma_bf16<0, 1>(wv[CUR][t][u], xq[t][q], acc[2 * u][2 * q + 1]);
-                        acc[2 * u + 1][2 * q] = fma_bf16<1, 0>(wv[CUR][t][u], xq[t][q], acc[2 * u + 1][2 * q]);
-                        acc[2 * u + 1][2 * q + 1] = fma_bf16<1, 1>(wv[CUR][t][u], xq[t][q], acc[2 * u + 1][2 * q + 1]);
-                    }
-        } else if constexpr (KN) {
+        if constexpr (KN) {
 #pragma unroll
             for (int t = 0; t < 4; ++t)                               // k-row of the lane: x word t >> 1, half t & 1
 #pragma unroll
@@ -262,23 +249,6 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
                             acc[2 * u + 1][mm] = fma_bf16<1, 0>(wv[CUR][t][u], xv[mm][t >> 1], acc[2 * u + 1][mm]);
                         }
                     }
-        } else if constexpr (XT) {
-#pragma unroll
-            for (int p = 0; p < 4; ++p)
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e)
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) {
-                            if (e == 0) {
-                                acc[j][2 * q] = fma_bf16<0, 0>(wv[CUR][j][p], xq[2 * p][q], acc[j][2 * q]);
-                                acc[j][2 * q + 1] = fma_bf16<0, 1>(wv[CUR][j][p], xq[2 * p][q], acc[j][2 * q + 1]);
-                            } else {
-                                acc[j][2 * q] = fma_bf16<1, 0>(wv[CUR][j][p], xq[2 * p + 1][q], acc[j][2 * q]);
-                                acc[j][2 * q + 1] = fma_bf16<1, 1>(wv[CUR][j][p], xq[2 * p + 1][q], acc[j][2 * q + 1]);
-                            }
-                        }
         } else {
 #pragma unroll
             for (int p = 0; p < 4; ++p)                               // word p = k-values 2p, 2p + 1 of the chunk
@@ -315,7 +285,7 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
     }
     asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
     ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
-    const int mm = threadIdx.x >> 4, col = (threadIdx.x & 15) * 4;    // 128 threads x 4 outputs = 8 rows x 64 columns
+    const int mm = threadIdx.x >> 4, col = (threadIdx.x & 15) * 4;    // 16 threads x 4 outputs per row of 64 columns
     if (mm < m && mm < MR && n0 + col < n) {
         float4 sum = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
@@ -334,37 +304,126 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
     }
 }
 
-template <int MR, bool KN>
-static cudaError_t launch_gemv(const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int m, int n, int k,
-                               int nslots, size_t smem, int blocks, cudaStream_t s)
+// ---------------------------------------------------------------------------------------------------------------------
+// (2) Warp-MMA path, 5 <= m <= 16.  NT: batch tiles of 8 rows (1 or 2).
+// Fragment layouts (PTX ISA, mma.m16n8k16, g = lane / 4, t = lane % 4): A regs = (row g | g+8) x (k 2t,2t+1 | +8);
+// B regs = (k 2t,2t+1 | +8) x (column g); D regs = (row g | g+8) x (columns 2t, 2t+1).  Here "row" is the output
+// column n of the GEMV (W tile) and "column" is the batch row.
+// ---------------------------------------------------------------------------------------------------------------------
+template <int NT, bool KN>
+__global__ void __launch_bounds__(GV_THREADS, 2)
+gemv_mma_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CUtensorMap xmap, uint16_t *__restrict__ y,
+                int64_t ldy, int m, int n, int k, int nslots)
 {
-    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
-    if (attr_gen != device_generation()) {
-        cudaError_t e = cudaFuncSetAttribute(gemv_kernel<MR, KN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS));
+    constexpr int SLOT = gemv_slot_bytes(8 * NT);
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *smem;
+    const GemvBars b = gemv_setup<SLOT>(smem_raw, nslots, &smem);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int n0 = blockIdx.x * GV_COLS;
+    const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+
+    if (warp == GV_CWARPS) {
+        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, nstages, nslots);
+        return;
+    }
+
+    // ldmatrix row addresses of this lane inside a slot, for k-step 0 (k-step ks adds a_step * ks, XOR-free: see below).
+    // NK: slot row = column (128 B = 64 k, 16-byte chunk c stored at c ^ (row & 7)).  Matrix j = lane >> 3:
+    //     rows 16w + (j & 1) * 8 + (lane & 7), chunk 2 ks + (j >> 1)  ->  a0..a3 in order.
+    // KN: slot row = k (128 B = 64 columns).  Matrix j: k-rows 16 ks + (j >> 1) * 8 + (lane & 7), chunk 2w + (j & 1),
+    //     read transposed; (krow & 7) = lane & 7 for every ks, so the swizzled chunk is a constant.
+    const int j4 = lane >> 3, r8 = lane & 7;
+    uint32_t a_off;
+    if (KN) a_off = (uint32_t)((j4 >> 1) * 8 + r8) * 128u + (uint32_t)(((2 * warp + (j4 & 1)) ^ r8) << 4);
+    else a_off = (uint32_t)(16 * warp + (j4 & 1) * 8 + r8) * 128u;
+    // X: slot row = batch row (128 B = 64 k, 128-byte swizzle).  One ldmatrix.x4 = chunks 4 kp + j of rows 0..7: the B
+    // fragments (b0, b1) of k-steps 2 kp and 2 kp + 1.
+    const uint32_t x_off = GV_W_BYTES + (uint32_t)r8 * 128u;
+
+    float acc[2][NT][4];
+#pragma unroll
+    for (int e = 0; e < 2; ++e)
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[e][t][c] = 0.f;
+
+    int slot = 0;
+    uint32_t par = 0;
+    for (int s = 0; s < nstages; ++s) {
+        ptx::mbar_wait(b.full0 + 8 * slot, par);
+        const uint32_t base = b.ring + slot * SLOT;
+        uint32_t af[4][4], bf[NT][2][4];
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+            if constexpr (KN) ldmatrix_x4<true>(af[ks], base + a_off + ks * 2048);
+            else ldmatrix_x4<false>(af[ks], base + a_off + (uint32_t)(((2 * ks + (j4 >> 1)) ^ r8) << 4));
+        }
+#pragma unroll
+        for (int t = 0; t < NT; ++t)
+#pragma unroll
+            for (int kp = 0; kp < 2; ++kp) ldmatrix_x4<false>(bf[t][kp], base + x_off + t * 1024 + (uint32_t)(((4 * kp + j4) ^ r8) << 4));
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(b.empty0 + 8 * slot);        // this stage's fragments are in registers: free the slot
+        if (++slot == nslots) { slot = 0; par ^= 1; }
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks)
+#pragma unroll
+            for (int t = 0; t < NT; ++t) mma_16816(acc[ks & 1][t], af[ks], bf[t][ks >> 1][2 * (ks & 1)], bf[t][ks >> 1][2 * (ks & 1) + 1]);
+    }
+
+    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
+    const int g = lane >> 2, t4 = lane & 3;
+#pragma unroll
+    for (int t = 0; t < NT; ++t)
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {                                 // D rows g, g + 8 = output columns
+            const int col = n0 + 16 * warp + g + 8 * h;
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {                             // D columns 2t, 2t + 1 = batch rows
+                const int row = 8 * t + 2 * t4 + e;
+                if (col < n && row < m)
+                    y[(int64_t)row * ldy + col] =
+                        __bfloat16_as_ushort(__float2bfloat16_rn(acc[0][t][2 * h + e] + acc[1][t][2 * h + e]));
+            }
+        }
+}
+
+template <typename Kernel>
+static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y,
+                               int64_t ldy, int m, int n, int k, int nslots, int blocks, cudaStream_t s)
+{
+    if (*attr_gen != device_generation()) {       // per-device function attribute: redo after tri_init() moved to another device
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS, 16));
         if (e != cudaSuccess) return e;
-        attr_gen = device_generation();
+        *attr_gen = device_generation();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(blocks);
     cfg.blockDim = dim3(GV_THREADS);
-    cfg.dynamicSmemBytes = smem;
+    cfg.dynamicSmemBytes = gemv_smem_bytes(nslots, xrows);
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, gemv_kernel<MR, KN>, wmap, xmap, y, ldy, m, n, k, nslots);
+    return cudaLaunchKernelEx(&cfg, kernel, wmap, xmap, y, ldy, m, n, k, nslots);
 }
 
+// Row-count dispatch.  One static generation counter per instantiation (function attributes are per device).
 template <bool KN>
-static cudaError_t launch_gemv_rows(int mr, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
-                                    int nslots, size_t smem, int blocks, cudaStream_t s)
+static cudaError_t launch_gemv_rows(int m, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
+                                    int nslots, int blocks, cudaStream_t s)
 {
-    if (mr <= 1) return launch_gemv<1, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
-    if (mr <= 2) return launch_gemv<2, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
-    if (mr <= 4) return launch_gemv<4, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
-    return launch_gemv<8, KN>(wmap, xmap, y, ldy, mr, n, k, nslots, smem, blocks, s);
+    static int gen[5] = {-1, -1, -1, -1, -1};
+    if (m <= 1) return launch_gemv(gemv_kernel<1, KN>, &gen[0], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
+    if (m <= 2) return launch_gemv(gemv_kernel<2, KN>, &gen[1], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
+    if (m <= 4) return launch_gemv(gemv_kernel<4, KN>, &gen[2], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
+    if (m <= 8) return launch_gemv(gemv_mma_kernel<1, KN>, &gen[3], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
+    return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
 }
 
 static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
@@ -393,46 +452,29 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
     const int blocks = (n + GV_COLS - 1) / GV_COLS;
     const bool kn = w_layout == TRI_W_KN;
 
-    CUtensorMap wmap;
-    if (kn) st = make_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, GV_COLS, GV_STAGE_K, CU_TENSOR_MAP_SWIZZLE_128B);
-    else st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
+    // Tensor maps (cached: re-encoding two maps costs more host time than the launch).  W: 64 x 64 boxes, 128-byte
+    // swizzle.  X: rows beyond m and k-values beyond k arrive as zeros; the MMA path reads it with ldmatrix, so its box
+    // is swizzled like W's; the FHFMA path reads plain rows.
+    CUtensorMap wmap, xmap;
+    if (kn) st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, GV_COLS, GV_STAGE_K, CU_TENSOR_MAP_SWIZZLE_128B);
+    else st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (st != TRI_OK) return st;
+    const int xrows = m <= 8 ? 8 : 16;
+    st = cached_tmap_2d_bf16(&xmap, x, (uint64_t)k, (uint64_t)m, (uint64_t)ldx * 2, GV_STAGE_K, xrows,
+                             m <= 4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
 
-    // Ring depth: 10 slots of 9 KiB per CTA (160 KiB of weights in flight per SM with two CTAs resident).  Measured on the
-    // config-3 shape: 8 -> 10 slots takes m = 1 from 21.6 to 20.1 us, m = 4 from 22.9 to 21.2, m = 8 (NK) from 36.6 to 28.3.
-    // Ten slots also fill the SM with two CTAs, so that no CTA of the NEXT call (programmatic dependent launch) moves in
-    // early and spins on its barriers in the issue slots of the running ones; 12 is no better.  KN with 5..8 rows likes 8.
-    // The partial-sum sets reuse the ring, so it is never smaller than they are.  TRI_GEMV_SLOTS is a debug override.
-    static int slots_cfg = -1;
-    if (slots_cfg < 0) {
-        const char *e = getenv("TRI_GEMV_SLOTS");
-        slots_cfg = e ? atoi(e) : 0;
-        if (slots_cfg < 4 || slots_cfg > GV_MAX_SLOTS) slots_cfg = 0;
-    }
-    const int nslots = slots_cfg ? slots_cfg : (kn && m > 4 ? 8 : 10);
-    static int force_fhfma = -1;                                     // debug only: TRI_GEMV_FHFMA=1 keeps every shape on this kernel
-    if (force_fhfma < 0) {
-        const char *e = getenv("TRI_GEMV_FHFMA");
-        force_fhfma = e ? atoi(e) : 0;
-    }
-    const size_t smem = gemv_smem_bytes(nslots);
-    static_assert((size_t)4 * GV_SLOT_BYTES >= (size_t)16 * GV_RED_STRIDE * 4, "the partial sums must fit the smallest ring");
+    // Ring depth: 10 slots of 9-10 KiB per CTA (160 KiB of weights in flight per SM with two CTAs resident).  Measured on
+    // the config-3 shape with the FHFMA path: 8 -> 10 slots takes m = 1 from 21.6 to 20.1 us, m = 4 from 22.9 to 21.2.  Ten
+    // slots also fill the SM with two CTAs, so that no CTA of the NEXT call (programmatic dependent launch) moves in early
+    // and spins on its barriers in the issue slots of the running ones.  The FHFMA path's partial-sum sets reuse the ring.
+    const int nslots = GV_MAX_SLOTS;
+    static_assert((size_t)GV_MAX_SLOTS * gemv_slot_bytes(8) >= (size_t)16 * GV_RED_STRIDE * 4, "the partial sums must fit the ring");
+    static_assert(2 * gemv_smem_bytes(GV_MAX_SLOTS, 16) <= 227 * 1024, "two CTAs per SM");
 
-    for (int r0 = 0; r0 < m; r0 += GV_M) {
-        const int mr = m - r0 < GV_M ? m - r0 : GV_M;
-        if (!kn && mr > 4 && k <= GEMV_NK8_KMAX && !force_fhfma) {       // FFMA2 kernel: see decode_gemv_m8.cu for why
-            st = launch_gemv_nk8(mr, n, k, x + (int64_t)r0 * ldx, ldx, w, ldw, y + (int64_t)r0 * ldy, ldy, di, s);
-            if (st != TRI_OK) return st;
-            continue;
-        }
-        CUtensorMap xmap;            // X rows r0 .. r0 + mr - 1; the 8-row box is zero-filled beyond them and beyond k
-        st = make_tmap_2d_bf16(&xmap, x + (int64_t)r0 * ldx, (uint64_t)k, (uint64_t)mr, (uint64_t)ldx * 2, GV_STAGE_K, GV_M,
-                               CU_TENSOR_MAP_SWIZZLE_NONE);
-        if (st != TRI_OK) return st;
-        cudaError_t e = kn ? launch_gemv_rows<true>(mr, wmap, xmap, y + (int64_t)r0 * ldy, ldy, n, k, nslots, smem, blocks, s)
-                           : launch_gemv_rows<false>(mr, wmap, xmap, y + (int64_t)r0 * ldy, ldy, n, k, nslots, smem, blocks, s);
-        if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "decode_gemv launch: %s", cudaGetErrorString(e));
-    }
+    cudaError_t e = kn ? launch_gemv_rows<true>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, s)
+                       : launch_gemv_rows<false>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, s);
+    if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "decode_gemv launch: %s", cudaGetErrorString(e));
     return TRI_OK;
 }
 

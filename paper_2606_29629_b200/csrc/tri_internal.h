@@ -31,10 +31,10 @@ int ensure_init(const DeviceInfo **info);
 int make_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer,
                       uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz);
 
-// decode_gemv_m8.cu: the FFMA2 kernel for TRI_W_NK, 5..8 rows, k <= GEMV_NK8_KMAX (x, y offset to the first row).
-constexpr int GEMV_NK8_KMAX = 4096;
-int launch_gemv_nk8(int mr, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, uint16_t *y,
-                    int64_t ldy, const DeviceInfo *di, cudaStream_t s);
+// The same through a small cache keyed on every argument (a tensor map depends on nothing else, so an entry can never
+// be stale): a decode_gemv / prefill_gemm call on buffers it has seen before encodes nothing.  Copies the map out.
+int cached_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer,
+                        uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz);
 
 inline bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 

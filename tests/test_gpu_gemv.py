@@ -68,8 +68,8 @@ def test_config3_full_output(layout):
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
 @pytest.mark.parametrize("m", [1, 4, 5, 16])
 def test_config3_shape_other_batch_sizes(layout, m):
-    """The config-3 weight matrix at the other decode batch sizes: m = 1, 4 run the FHFMA kernel in
-    both layouts, m = 5 the FFMA2 kernel with zero-filled rows, m = 16 two launches of 8 rows; full output, stated bound."""
+    """The config-3 weight matrix at the other decode batch sizes: m = 1, 4 run the FHFMA kernels,
+    m = 5 the warp-MMA kernel with zero-filled rows, m = 16 its two-tile form; full output, stated bound."""
     k, n = 3584, 18944
     x = normal_bf16(2, (m, k), 1.0, stream=7)
     w = normal_bf16(2, (k, n), 0.02, stream=1)
@@ -79,31 +79,47 @@ def test_config3_shape_other_batch_sizes(layout, m):
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
-def test_identity_and_permutation_are_exact(layout):
+@pytest.mark.parametrize("m", [5, 8, 16])
+def test_down_projection_shape_full_output(layout, m):
+    """The Thinker MLP down-projection at decode batch sizes (18944 -> 3584): K = 18944 = 296 stages
+    through the 10-slot ring, every row count of the warp-MMA path; full output, stated bound."""
+    k, n = 18944, 3584
+    x = normal_bf16(2, (m, k), 1.0, stream=8)
+    w = normal_bf16(2, (k, n), 0.02, stream=9)
+    wp = phys_w(w, layout)
+    y = run_gemv(x, wp, m, n, k, layout)
+    assert check_against_oracle(y, x, wp, layout, stated=True) < 1.0
+
+
+@pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
+@pytest.mark.parametrize("m", [1, 3, 4, 8, 11, 16])            # FHFMA kernels (1, 2, 4 rows) and the MMA kernel (1 and 2 batch tiles)
+def test_identity_and_permutation_are_exact(layout, m):
     k = n = 256
-    x = normal_bf16(21, (8, k))
+    x = normal_bf16(21, (m, k))
     eye = f32_to_bf16_bits(np.eye(k, dtype=np.float32))
-    assert (run_gemv(x, phys_w(eye, layout), 8, n, k, layout) == x).all()
+    assert (run_gemv(x, phys_w(eye, layout), m, n, k, layout) == x).all()
     pi = np.random.default_rng(3).permutation(k)
     wl = np.zeros((k, n), np.float32)
     wl[pi, np.arange(n)] = 1.0                                   # Y[:, j] = X[:, pi(j)]
-    y = run_gemv(x, phys_w(f32_to_bf16_bits(wl), layout), 8, n, k, layout)
+    y = run_gemv(x, phys_w(f32_to_bf16_bits(wl), layout), m, n, k, layout)
     assert (y == x[:, pi]).all()
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
+@pytest.mark.parametrize("m", [2, 8, 13])
 @pytest.mark.parametrize("k", [16, 256, 3584])
-def test_ones_give_k_exactly(layout, k):
+def test_ones_give_k_exactly(layout, m, k):
     n = 136
-    ones_x = np.full((8, k), 0x3F80, np.uint16)
+    ones_x = np.full((m, k), 0x3F80, np.uint16)
     ones_w = np.full((k, n), 0x3F80, np.uint16)
-    y = run_gemv(ones_x, phys_w(ones_w, layout), 8, n, k, layout)
+    y = run_gemv(ones_x, phys_w(ones_w, layout), m, n, k, layout)
     assert (bf16_bits_to_f32(y) == float(k)).all()
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
 @pytest.mark.parametrize("m,n,k", [(1, 8, 8), (7, 264, 80), (8, 1000, 136), (9, 129, 264), (16, 520, 4096),
-                                   (3, 18944, 128), (8, 127, 3584), (2, 72, 18944), (4, 200, 8200), (5, 64, 64), (12, 65, 72)])
+                                   (3, 18944, 128), (8, 127, 3584), (2, 72, 18944), (4, 200, 8200), (5, 64, 64), (12, 65, 72),
+                                   (5, 200, 4104), (8, 136, 8200), (6, 72, 18944), (13, 200, 4104), (16, 72, 8200), (10, 3, 24)])
 def test_ragged_shapes(layout, m, n, k):
     x = normal_bf16(30 + m, (m, k))
     w = normal_bf16(31 + m, (k, n), 0.05)
