@@ -374,10 +374,16 @@ def compact_line(full):
     if full.get("energy"):
         out["j_per_flop"] = sig(full["energy"].get("j_per_flop"), 3)
     out["detail"] = DETAIL_FILE
-    for k in ("value", "ms_per_step", "min_frac"):
-        if isinstance(out.get(k), float):
-            out[k] = sig(out[k], 6)
-    return json.dumps(out, separators=(",", ":"))
+
+    def rounded(x):                                                   # 6 significant digits are plenty on the line; the file has them all
+        if isinstance(x, float):
+            return sig(x, 6)
+        if isinstance(x, dict):
+            return {k: rounded(v) for k, v in x.items()}
+        if isinstance(x, list):
+            return [rounded(v) for v in x]
+        return x
+    return json.dumps(rounded(out), separators=(",", ":"))
 
 
 def emit(full):

@@ -117,20 +117,14 @@ static int run(unsigned k, float a, float b, size_t n, const float *in, float *o
     int st = ensure_init(nullptr);
     if (st != TRI_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    static int variant = -1;                                 // debug override only: TRI_FMA_VEC in {1, 2, 4, 8}
-    if (variant < 0) {
-        const char *e = getenv("TRI_FMA_VEC");
-        variant = e ? atoi(e) : 0;
-    }
     // float4 loads in flight per thread (= 4 x VEC chains), chosen by measurement on B200 (N = 2^28): the memory-bound
     // end likes many small blocks (VEC 2: 6.85 TB/s), the ridge needs both the load queue and the FP32 pipe full
     // (VEC 4 at k = 32, VEC 8 from k = 40: 1.04 of the HBM roof there instead of 0.96, 0.95-0.98 of the ALU roof from k = 48
     // instead of 0.90-0.96; VEC 16 is no better), the far compute-bound end
     // is indifferent (VEC 2: 0.998).
-    int vec = variant ? variant : (k <= 24 ? 2 : k <= 35 ? 4 : k < 2048 ? 8 : 2);
+    const int vec = k <= 24 ? 2 : k <= 35 ? 4 : k < 2048 ? 8 : 2;
     cudaError_t e;
     switch (vec) {
-        case 1: e = launch<1>(in, out, n, k, a, b, s); break;
         case 2: e = launch<2>(in, out, n, k, a, b, s); break;
         case 8: e = launch<8>(in, out, n, k, a, b, s); break;
         default: e = launch<4>(in, out, n, k, a, b, s); break;

@@ -13,7 +13,9 @@ static std::mutex g_mu;
 static void *g_lib = nullptr;
 static Api g_api;
 static bool g_tried = false;
-static bool g_locked_by_us[64] = {false};
+static Device g_locked_handle[64] = {nullptr};   // by CUDA ordinal: the NVML handle the lock was taken through (ordinals differ
+                                                    // from NVML indices under CUDA_VISIBLE_DEVICES, so unload() must not re-derive it)
+static int g_active_tracers = 0;                    // sampler threads using g_api; unload() waits for none
 
 template <typename F>
 static bool sym(F &f, const char *name, const char *alt = nullptr)
@@ -86,18 +88,28 @@ Device device_handle(int device)
     return h;
 }
 
-void unload()
+void tracer_enter()
 {
     std::lock_guard<std::mutex> lk(g_mu);
+    ++g_active_tracers;
+}
+
+void tracer_leave()
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    --g_active_tracers;
+}
+
+bool unload()
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g_active_tracers > 0) return false;       // a sampler thread is inside NVML: keep the library mapped
     if (g_api.ok) {
         for (int d = 0; d < 64; ++d)
-            if (g_locked_by_us[d]) {
-                Device h = nullptr;
-                if (g_api.device_by_index((unsigned)d, &h) == SUCCESS) {
-                    if (g_api.reset_gpu_locked) g_api.reset_gpu_locked(h);
-                    if (g_api.reset_mem_locked) g_api.reset_mem_locked(h);
-                }
-                g_locked_by_us[d] = false;
+            if (g_locked_handle[d]) {
+                if (g_api.reset_gpu_locked) g_api.reset_gpu_locked(g_locked_handle[d]);
+                if (g_api.reset_mem_locked) g_api.reset_mem_locked(g_locked_handle[d]);
+                g_locked_handle[d] = nullptr;
             }
         g_api.shutdown();
         g_api = Api();
@@ -107,6 +119,7 @@ void unload()
         g_lib = nullptr;
     }
     g_tried = false;
+    return true;
 }
 
 int read_sample(const Api *a, Device h, tri_sample *s, bool with_energy)
@@ -124,6 +137,7 @@ int read_sample(const Api *a, Device h, tri_sample *s, bool with_energy)
 
 }  // namespace nvml
 void release_clock_scratch();
+void release_splitk_workspaces();
 }  // namespace tri
 
 extern "C" {
@@ -151,7 +165,7 @@ int tri_lock_clocks(int device, unsigned sm_mhz, unsigned mem_mhz)
     int r = a->set_gpu_locked(h, sm_mhz, sm_mhz);
     if (r == tri::nvml::ERROR_NO_PERMISSION) return tri::fail(TRI_ERR_NO_PERMISSION, "nvmlDeviceSetGpuLockedClocks: %s", a->error_string(r));
     if (r != tri::nvml::SUCCESS) return tri::fail(TRI_ERR_NVML_UNAVAILABLE, "nvmlDeviceSetGpuLockedClocks: %s", a->error_string(r));
-    tri::nvml::g_locked_by_us[device] = true;
+    tri::nvml::g_locked_handle[device] = h;
     if (mem_mhz && a->set_mem_locked) {
         r = a->set_mem_locked(h, mem_mhz, mem_mhz);
         if (r == tri::nvml::ERROR_NO_PERMISSION) return tri::fail(TRI_ERR_NO_PERMISSION, "nvmlDeviceSetMemoryLockedClocks: %s", a->error_string(r));
@@ -169,7 +183,7 @@ int tri_reset_clocks(int device)
     if (!h) return TRI_ERR_NVML_UNAVAILABLE;
     int r = a->reset_gpu_locked ? a->reset_gpu_locked(h) : tri::nvml::ERROR_NOT_SUPPORTED;
     if (a->reset_mem_locked) a->reset_mem_locked(h);
-    tri::nvml::g_locked_by_us[device] = false;
+    tri::nvml::g_locked_handle[device] = nullptr;
     if (r == tri::nvml::ERROR_NO_PERMISSION) return tri::fail(TRI_ERR_NO_PERMISSION, "nvmlDeviceResetGpuLockedClocks: %s", a->error_string(r));
     if (r != tri::nvml::SUCCESS) return tri::fail(TRI_ERR_NVML_UNAVAILABLE, "nvmlDeviceResetGpuLockedClocks: %s", a->error_string(r));
     return TRI_OK;
@@ -177,7 +191,10 @@ int tri_reset_clocks(int device)
 
 void tri_shutdown(void)
 {
+    // With a phase trace still running NVML stays loaded (its sampler thread is inside it) and clocks this process locked
+    // stay locked until the trace has been stopped and tri_shutdown() is called again.
     tri::nvml::unload();
+    tri::release_splitk_workspaces();
     tri::release_clock_scratch();
 }
 

@@ -35,7 +35,11 @@ struct Api {
 const Api *api();
 // NVML handle of CUDA device `device` (matched through its PCI bus id); nullptr on failure.
 Device device_handle(int device);
-void unload();
+// Resets clocks locked through tri_lock_clocks (by the handle they were locked through) and unloads NVML; false (and
+// nothing done) while a sampler thread is registered.
+bool unload();
+void tracer_enter();
+void tracer_leave();
 // Fills the NVML fields of *s (t_s and phase are left to the caller).
 // with_energy = false skips nvmlDeviceGetTotalEnergyConsumption (measured on B200: 4 ms idle, 10-13 ms under load, against
 // microseconds for the other queries) and leaves s->energy_mj untouched.

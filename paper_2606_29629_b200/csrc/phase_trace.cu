@@ -129,6 +129,7 @@ int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t ca
     t->cap = cap;
     t->period_us = period_us;
     t->t0 = tri::now_s();
+    tri::nvml::tracer_enter();                    // tri_shutdown() keeps NVML loaded while this sampler runs
     t->th = std::thread([t] { t->run(); });
     *handle = t;
     return TRI_OK;
@@ -147,6 +148,7 @@ int phase_trace_stop(void *handle, size_t *n_samples)
     tri::Tracer *t = static_cast<tri::Tracer *>(handle);
     t->stop.store(true, std::memory_order_release);
     if (t->th.joinable()) t->th.join();
+    tri::nvml::tracer_leave();
     if (n_samples) *n_samples = t->n.load();
     bool ovf = t->overflow;
     delete t;
@@ -177,15 +179,29 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
     if (!h) return TRI_ERR_NVML_UNAVAILABLE;
 
     cudaStream_t s = static_cast<cudaStream_t>(wl->stream);
-    cudaEvent_t e0, e1, ring[2];
-    TRI_CUDA(cudaEventCreate(&e0));
-    TRI_CUDA(cudaEventCreate(&e1));
-    TRI_CUDA(cudaEventCreateWithFlags(&ring[0], cudaEventDisableTiming));
-    TRI_CUDA(cudaEventCreateWithFlags(&ring[1], cudaEventDisableTiming));
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};      // e0, e1 (timed), ring[0..1] (queue depth)
+    auto destroy_events = [&ev] {
+        for (cudaEvent_t &e : ev)
+            if (e) {
+                cudaEventDestroy(e);
+                e = nullptr;
+            }
+    };
+    for (int i = 0; i < 4; ++i) {
+        cudaError_t ce = i < 2 ? cudaEventCreate(&ev[i]) : cudaEventCreateWithFlags(&ev[i], cudaEventDisableTiming);
+        if (ce != cudaSuccess) {
+            destroy_events();
+            return fail(TRI_ERR_CUDA, "cudaEventCreate: %s", cudaGetErrorString(ce));
+        }
+    }
+    cudaEvent_t e0 = ev[0], e1 = ev[1], ring[2] = {ev[2], ev[3]};
 
     void *handle = nullptr;
     st = phase_trace_start(di->device, period_ms * 1000u, samples, cap, &handle);
-    if (st != TRI_OK) return st;
+    if (st != TRI_OK) {
+        destroy_events();
+        return st;
+    }
     Tracer *tr = static_cast<Tracer *>(handle);
     const double t0 = tr->t0;
 
@@ -283,10 +299,7 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
         q->j_per_token = q->tokens > 0 ? q->energy_j / q->tokens : 0.0;
     }
     *n_summaries = nsum;
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaEventDestroy(ring[0]);
-    cudaEventDestroy(ring[1]);
+    destroy_events();
     if (status != TRI_OK) return status;
     if (st2 != TRI_OK) return st2;
     if (truncated) return fail(TRI_ERR_BUFFER_TOO_SMALL, "summary buffer full; later phases dropped");

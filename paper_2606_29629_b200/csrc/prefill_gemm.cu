@@ -1,44 +1,40 @@
 // a3. Prefill-phase GEMM ("dense GEMM kernels"; BASELINE.json config 4; ABI in
 // include/triroof.h):   C[m][n] = bf16_rne( sum_k A[m][k] * W[k][n] ),  fp32 accumulation in TMEM.
 //
-// The only tensor-core path of the library (a dense contraction).  Persistent, warp-specialised
-// tcgen05 kernel, one CTA per SM:
-//   warp 0   TMA producer   one elected lane: cp.async.bulk.tensor loads of the A tile (128 x 64) and the
-//                           W tile (256 x 64) into a 4-stage ring (48 KiB per stage, 128-byte swizzle),
-//                           completion on the stage's "full" mbarrier
-//   warp 1   MMA issuer     one elected lane: per 64-wide k-block four tcgen05.mma.kind::f16
-//                           (M 128, N 256, K 16) accumulating fp32 in tensor memory; tcgen05.commit
-//                           releases the stage ("empty") and, after the last k-block, publishes the
-//                           accumulator ("tmem_full")
-//   warp 2   TMEM owner     allocates all 512 columns = two 128 x 256 fp32 accumulators, so the epilogue
-//                           of tile t overlaps the main loop of tile t+1
-//   warps 4-7 epilogue      tcgen05.ld (lane = row, 32 columns at a time) -> cvt.rn.bf16x2 -> 16-byte
-//                           global stores; releases the accumulator ("tmem_empty")
-// Tile order: tile = blockIdx.x + i * gridDim.x with the M index fastest, so the CTAs of a wave share
-// W panels through L2 while A (29 MB) stays L2 resident.  4096 x 18944 gives 32 x 74 = 2368 tiles =
-// 148 SMs x 16: no wave quantisation.  Ragged M / N / K: TMA zero-fills out-of-bounds reads; stores clip.
+// The only tcgen05 path of the library (a dense contraction).  This file holds the entry point, its dispatch, and the
+// one-CTA kernel used when A has at most 128 rows; m > 128 goes to the CTA-pair kernel of prefill_gemm_2sm.cu (256 x 256
+// pair tiles), which a short A would leave three quarters empty.
 //
-// W layouts: TRI_W_NK is the K-major B operand (canonical).  TRI_W_KN is the MN-major B operand: the
-// W tile is loaded as four 64(n) x 64(k) boxes and described to the MMA with the MN-major descriptor.
+// One-CTA kernel (m <= 128: chunked-prefill tails, speculative / large-batch decode): weight-streaming bound, so the
+// tile is 128 x 128 — 148 tiles for n = 18944, one per SM — and when there are fewer tiles than SMs every tile is cut
+// along K into `parts` ranges (gemm_common.cuh next_work / splitk_*) so that all SMs pull on HBM.  Warp roles as in the
+// pair kernel: warp 0 TMA producer (A 128 x 64 and W 128 x 64 per k-block into a 6-stage ring, 128-byte swizzle), warp 1
+// MMA issuer (tcgen05.mma.cta_group::1.kind::f16, M 128, N 128, K 16), warp 2 TMEM owner (two 128-column accumulators),
+// warps 4-7 epilogue (tcgen05.ld -> cvt.rn.bf16x2 -> 16-byte global stores; the output is small here).
+// Ragged M / N / K: TMA zero-fills out-of-bounds reads; stores clip.
+//
+// W layouts: TRI_W_NK is the K-major B operand (canonical).  TRI_W_KN is the MN-major B operand: the W tile is loaded
+// as 64(n) x 64(k) boxes and described to the MMA with the MN-major descriptor.
 #include "tri_internal.h"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
 
-#include <cstdlib>
+#include <mutex>
+#include <vector>
 
 namespace tri {
 
-constexpr int GM_BM = 128, GM_BN = 256, GM_BK = 64;
-constexpr int GM_STAGES = 4;
+constexpr int GM_BM = 128, GM_BN = 128, GM_BK = 64;
+constexpr int GM_STAGES = 6;
 constexpr int GM_A_BYTES = GM_BM * GM_BK * 2;      // 16 KiB
-constexpr int GM_B_BYTES = GM_BN * GM_BK * 2;      // 32 KiB
+constexpr int GM_B_BYTES = GM_BN * GM_BK * 2;      // 16 KiB
 constexpr int GM_STAGE_BYTES = GM_A_BYTES + GM_B_BYTES;
 constexpr int GM_THREADS = 256;
-constexpr int GM_TMEM_COLS = 512;
+constexpr int GM_TMEM_COLS = 2 * GM_BN;
 constexpr int GM_SMEM_BYTES = 1024 + GM_STAGES * GM_STAGE_BYTES + 256;
 
 __global__ void __launch_bounds__(GM_THREADS, 1)
-gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap, const GemmParams p)
+gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap, const GemmParams p)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -49,8 +45,9 @@ gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CU
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + GM_STAGES * GM_STAGE_BYTES + 16 * GM_STAGES + 32);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int ntiles = p.tiles_m * p.tiles_n;
+    const int ntiles = p.tiles_m * p.tiles_n, me = blockIdx.x, nw = gridDim.x;
 
+    if (p.parts > 1) ptx::pdl_launch_dependents();        // splitk_reduce_kernel may take its place; it waits for this grid
     if (threadIdx.x == 0) {
         for (int s = 0; s < GM_STAGES; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);
@@ -76,23 +73,24 @@ gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CU
         if (ptx::elect_one()) {
             ptx::prefetch_tmap(&amap);
             ptx::prefetch_tmap(&wmap);
-            const uint64_t pol_w = ptx::policy_evict_first();
-            const uint64_t pol_a = ptx::policy_evict_last();
+            const uint64_t pol_w = ptx::policy_evict_first();        // every W element is read exactly once
+            const uint64_t pol_a = ptx::policy_evict_last();         // A is re-read by every CTA
             uint32_t it = 0;
-            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-                const int tm = t % p.tiles_m, tn = t / p.tiles_m;
-                for (int kb = 0; kb < p.kblocks; ++kb, ++it) {
+            GemmWork wk;
+            for (int i = 0; next_work(p, ntiles, me, nw, i, wk); ++i) {
+                const int tm = wk.tile % p.tiles_m, tn = wk.tile / p.tiles_m;
+                for (int kb = wk.kb0; kb < wk.kb1; ++kb, ++it) {
                     const uint32_t s = it % GM_STAGES, ph = (it / GM_STAGES) & 1;
                     ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);
                     const uint32_t fb = full0 + 8 * s;
-                    ptx::mbar_arrive_expect_tx(fb, GM_STAGE_BYTES);
+                    ptx::mbar_arrive_expect_tx(fb, p.a_box_bytes + GM_B_BYTES);
                     const uint32_t sa = ring + s * GM_STAGE_BYTES, sb = sa + GM_A_BYTES;
                     ptx::tma_load_2d_hint(sa, &amap, kb * GM_BK, tm * GM_BM, fb, pol_a);
                     if (!p.b_mn_major) {
                         ptx::tma_load_2d_hint(sb, &wmap, kb * GM_BK, tn * GM_BN, fb, pol_w);
                     } else {
 #pragma unroll
-                        for (int q = 0; q < 4; ++q)   // four 64(n) x 64(k) boxes, 8 KiB each
+                        for (int q = 0; q < GM_BN / 64; ++q)   // 64(n) x 64(k) boxes, 8 KiB each
                             ptx::tma_load_2d_hint(sb + q * 8192, &wmap, tn * GM_BN + q * 64, kb * GM_BK, fb, pol_w);
                     }
                 }
@@ -103,12 +101,13 @@ gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CU
         if (ptx::elect_one()) {
             const uint32_t idesc = make_idesc(GM_BM, GM_BN, p.b_mn_major);
             uint32_t it = 0, tcount = 0;
-            for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++tcount) {
+            GemmWork wk;
+            for (int i = 0; next_work(p, ntiles, me, nw, i, wk); ++i, ++tcount) {
                 const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
                 ptx::mbar_wait(tempty0 + 8 * acc, aph ^ 1);          // epilogue has drained this accumulator
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * GM_BN;
-                for (int kb = 0; kb < p.kblocks; ++kb, ++it) {
+                for (int kb = wk.kb0; kb < wk.kb1; ++kb, ++it) {
                     const uint32_t s = it % GM_STAGES, ph = (it / GM_STAGES) & 1;
                     ptx::mbar_wait(full0 + 8 * s, ph);
                     ptx::tc_fence_after();
@@ -118,26 +117,42 @@ gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CU
 #pragma unroll
                     for (int kk = 0; kk < GM_BK / 16; ++kk)
                         ptx::mma_bf16_ss(d_tmem, adesc + (uint64_t)((kk * 32) >> 4), bdesc + (uint64_t)((kk * p.b_kstep) >> 4),
-                                         idesc, (kb | kk) != 0);
+                                         idesc, (kb > wk.kb0) | (kk != 0));
                     ptx::mma_commit(empty0 + 8 * s);                 // stage free once these MMAs retire
                 }
                 ptx::mma_commit(tfull0 + 8 * acc);                   // accumulator complete
             }
         }
     } else if (warp >= 4) {
-        // ===== epilogue: TMEM -> registers -> bf16 -> global =====
+        // ===== epilogue: TMEM -> registers (-> split-K sum through L2) -> bf16 -> global =====
         const int ew = warp & 3;                                      // TMEM lanes 32*ew .. 32*ew+31
         uint32_t tcount = 0;
-        for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++tcount) {
-            const int tm = t % p.tiles_m, tn = t / p.tiles_m;
+        GemmWork wk;
+        for (int i = 0; next_work(p, ntiles, me, nw, i, wk); ++i, ++tcount) {
+            const int tm = wk.tile % p.tiles_m, tn = wk.tile / p.tiles_m;
             const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
             ptx::mbar_wait(tfull0 + 8 * acc, aph);
             ptx::tc_fence_after();
             const int row = tm * GM_BM + ew * 32 + lane;
             const bool row_ok = row < p.m;
             uint16_t *crow = p.c + (int64_t)row * p.ldc + (int64_t)tn * GM_BN;
-            const int ncols = p.n - tn * GM_BN;                       // valid columns in this tile (may exceed 256)
+            const int ncols = p.n - tn * GM_BN;                       // valid columns in this tile (may exceed 128)
             const uint32_t taddr = tmem_base + acc * GM_BN + ((uint32_t)(ew * 32) << 16);
+            if (wk.split >= 0) {
+                // split tile: this warp's 32 x 128 slice of the CTA's partial sums goes to the workspace, nothing to C
+                float *slice = p.ws + ((size_t)(wk.split * p.parts + wk.part) * 4 + ew) * (32 * GM_BN);
+#pragma unroll 1
+                for (int cb = 0; cb < GM_BN / 32; ++cb) {
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32b_x32(taddr + cb * 32, r);
+                    ptx::tmem_ld_wait();
+                    splitk_put(slice, cb, lane, r);
+                }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(tempty0 + 8 * acc);
+                continue;
+            }
 #pragma unroll 1
             for (int cb = 0; cb < GM_BN / 32; ++cb) {
                 uint32_t r[32];
@@ -178,6 +193,142 @@ gemm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CU
     }
 }
 
+// ---- split-K: the sum of the parts ---------------------------------------------------------------------------------
+// One thread per float4 of a split tile (fragment order, see splitk_put): adds the `parts` partials in ascending order
+// (fixed: the result does not depend on which CTA finished first), rounds to bf16 and stores 4 outputs of one row.
+__global__ void __launch_bounds__(256)
+splitk_reduce_kernel(const GemmParams p, int tile_rows, int tile_cols, int pair_order)
+{
+    ptx::pdl_wait();                                       // the GEMM kernel's partial tiles are complete and visible
+    const int ntiles = p.tiles_m * p.tiles_n, nsplit = ntiles - p.full_tiles;
+    const int tile4 = tile_rows * tile_cols / 4;           // float4 per tile
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nsplit * tile4) return;
+    const int st = idx / tile4, f = idx - st * tile4;
+    const float4 *src = reinterpret_cast<const float4 *>(p.ws) + (size_t)st * p.parts * tile4 + f;
+    float4 sum = make_float4(0.f, 0.f, 0.f, 0.f);
+    int part = 0;
+    for (; part + 4 <= p.parts; part += 4) {               // four loads in flight
+        const float4 v0 = __ldcg(src + (size_t)part * tile4), v1 = __ldcg(src + (size_t)(part + 1) * tile4),
+                     v2 = __ldcg(src + (size_t)(part + 2) * tile4), v3 = __ldcg(src + (size_t)(part + 3) * tile4);
+        sum.x = ((((sum.x + v0.x) + v1.x) + v2.x) + v3.x);
+        sum.y = ((((sum.y + v0.y) + v1.y) + v2.y) + v3.y);
+        sum.z = ((((sum.z + v0.z) + v1.z) + v2.z) + v3.z);
+        sum.w = ((((sum.w + v0.w) + v1.w) + v2.w) + v3.w);
+    }
+    for (; part < p.parts; ++part) {
+        const float4 v = __ldcg(src + (size_t)part * tile4);
+        sum.x += v.x; sum.y += v.y; sum.z += v.z; sum.w += v.w;
+    }
+    int tm, tn;
+    const int t = p.full_tiles + st;
+    if (pair_order) tile_coords(p, t, tm, tn);
+    else { tm = t % p.tiles_m; tn = t / p.tiles_m; }
+    const int slice4 = 8 * tile_cols;                      // float4 per 32-row slice
+    const int slice = f / slice4, r = f - slice * slice4;
+    const int blk = r >> 8, q = (r >> 5) & 7, lane = r & 31;
+    const int row = tm * tile_rows + slice * 32 + lane, col = tn * tile_cols + blk * 32 + q * 4;
+    if (row >= p.m || col >= p.n) return;
+    uint16_t *dst = p.c + (int64_t)row * p.ldc + col;
+    const uint32_t lo = ptx::pack_bf16x2(sum.x, sum.y), hi = ptx::pack_bf16x2(sum.z, sum.w);
+    if (col + 4 <= p.n) {
+        *reinterpret_cast<uint2 *>(dst) = make_uint2(lo, hi);       // ldc % 8 == 0 and col % 4 == 0: 8-byte aligned
+    } else {
+        const uint16_t e[4] = {(uint16_t)lo, (uint16_t)(lo >> 16), (uint16_t)hi, (uint16_t)(hi >> 16)};
+        for (int c = 0; col + c < p.n; ++c) dst[c] = e[c];
+    }
+}
+
+int launch_splitk_reduce(const GemmParams &p, int tile_rows, int tile_cols, bool pair_order, cudaStream_t s)
+{
+    const int nsplit = p.tiles_m * p.tiles_n - p.full_tiles;
+    const long long threads = (long long)nsplit * tile_rows * tile_cols / 4;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((threads + 255) / 256));
+    cfg.blockDim = dim3(256);
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    TRI_CUDA(cudaLaunchKernelEx(&cfg, splitk_reduce_kernel, p, tile_rows, tile_cols, pair_order ? 1 : 0));
+    return TRI_OK;
+}
+
+// ---- split-K workspace, one per stream (calls on one stream are ordered, so they can share it) ------------------------
+struct SplitWs {
+    int generation;
+    cudaStream_t stream;
+    float *ws;
+    size_t ws_bytes;
+};
+static std::mutex g_ws_mu;
+static std::vector<SplitWs> g_ws;
+
+int splitk_workspace(cudaStream_t stream, size_t ws_bytes, float **ws)
+{
+    std::lock_guard<std::mutex> lk(g_ws_mu);
+    SplitWs *e = nullptr;
+    for (auto &x : g_ws)
+        if (x.stream == stream && x.generation == device_generation()) e = &x;
+    if (!e) {
+        if (g_ws.size() >= 64) return fail(TRI_ERR_CUDA, "split-K workspaces for more than 64 streams");
+        g_ws.push_back(SplitWs{device_generation(), stream, nullptr, 0});
+        e = &g_ws.back();
+    }
+    if (e->ws_bytes < ws_bytes) {
+        // grow: earlier calls on this stream may still be using the old buffer, so wait for the stream first
+        TRI_CUDA(cudaStreamSynchronize(stream));
+        if (e->ws) cudaFree(e->ws);
+        e->ws = nullptr;
+        e->ws_bytes = 0;
+        // 74 pair tiles of 256 x 256 fp32 (the most left x parts can be) = 19.4 MB covers every shape of either kernel
+        const size_t wb = ws_bytes < (size_t)(20u << 20) ? (size_t)(20u << 20) : ws_bytes;
+        TRI_CUDA(cudaMalloc(&e->ws, wb));
+        e->ws_bytes = wb;
+    }
+    *ws = e->ws;
+    return TRI_OK;
+}
+
+void release_splitk_workspaces()
+{
+    std::lock_guard<std::mutex> lk(g_ws_mu);
+    for (auto &x : g_ws)
+        if (x.ws) cudaFree(x.ws);
+    g_ws.clear();
+}
+
+static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, const GemmParams &p, int sm_count, cudaStream_t s)
+{
+    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen != device_generation()) {
+        TRI_CUDA(cudaFuncSetAttribute(gemm_1sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_BYTES));
+        attr_gen = device_generation();
+    }
+    GemmParams q = p;
+    const int ntiles = p.tiles_m * p.tiles_n;
+    const int left = ntiles % sm_count;
+    int parts = left ? sm_count / left : 1;
+    if (parts > p.kblocks) parts = p.kblocks;
+    q.full_tiles = ntiles;
+    q.parts = 1;
+    q.ws = nullptr;
+    int grid = ntiles < sm_count ? ntiles : sm_count;
+    if (parts >= 2 && (parts - 1) * p.kblocks >= 8 * parts) {        // the 128 x 128 fp32 partial is a quarter of the pair kernel's
+        q.full_tiles = ntiles - left;
+        q.parts = parts;
+        int st = splitk_workspace(s, (size_t)left * parts * GM_BM * GM_BN * sizeof(float), &q.ws);
+        if (st != TRI_OK) return st;
+        if (q.full_tiles == 0) grid = left * parts;
+    }
+    gemm_1sm_kernel<<<grid, GM_THREADS, GM_SMEM_BYTES, s>>>(amap, wmap, q);
+    TRI_CUDA(cudaGetLastError());
+    if (q.parts > 1) return launch_splitk_reduce(q, GM_BM, GM_BN, false, s);
+    return TRI_OK;
+}
+
 static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw, int w_layout,
                      uint16_t *c, int64_t ldc, void *stream)
 {
@@ -200,51 +351,40 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     int st = ensure_init(&di);
     if (st != TRI_OK) return st;
 
-    // Default: the CTA-pair kernel (prefill_gemm_2sm.cu).  TRI_GEMM_1SM=1 (debug / A-B comparison) keeps the one-CTA kernel.
-    static int one_sm = -1;
-    if (one_sm < 0) { const char *e = getenv("TRI_GEMM_1SM"); one_sm = e ? atoi(e) : 0; }
-    const int bn_box = one_sm ? GM_BN : GM_BN / 2;            // W columns staged per CTA
+    const bool one_sm = m <= GM_BM;                           // a short A: 128 x 128 tiles, one CTA each (see the file header)
     const int rows_per_tile = one_sm ? GM_BM : 2 * GM_BM;
+    const int cols_per_tile = one_sm ? GM_BN : 2 * GM_BN;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
 
+    // Both kernels stage A as 128-row x 64-k boxes and W as 128 columns x 64 k per CTA (cached maps)
+    // A box: 128 rows; for a short A only the rows that exist, rounded up to the 8-row swizzle atom (zero-filling 112
+    // absent rows per box made m = 16 slower than m = 64; the MMA still reads 128 rows, and what it computes from the
+    // stale rows lands in accumulator rows >= m, which are never stored)
+    const int a_rows = one_sm ? ((m + 7) / 8) * 8 : GM_BM;
     CUtensorMap amap, wmap;
-    st = make_tmap_2d_bf16(&amap, a, (uint64_t)k, (uint64_t)m, (uint64_t)lda * 2, GM_BK, GM_BM, CU_TENSOR_MAP_SWIZZLE_128B);
+    st = cached_tmap_2d_bf16(&amap, a, (uint64_t)k, (uint64_t)m, (uint64_t)lda * 2, GM_BK, a_rows, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
-    GemmParams p;
+    GemmParams p = {};
+    p.a_box_bytes = a_rows * GM_BK * 2;
     p.m = m; p.n = n; p.k = k;
     p.tiles_m = (m + rows_per_tile - 1) / rows_per_tile;
-    p.tiles_n = (n + GM_BN - 1) / GM_BN;
+    p.tiles_n = (n + cols_per_tile - 1) / cols_per_tile;
     p.kblocks = (k + GM_BK - 1) / GM_BK;
     p.ldc = ldc;
     p.c = c;
-    {
-        static int wpol = -1;                               // debug only: TRI_GEMM_WPOL in {0, 1, 2}
-        if (wpol < 0) { const char *e = getenv("TRI_GEMM_WPOL"); wpol = e ? atoi(e) : 2; }      // measured on config 4: evict-last 1.392 PFLOP/s sustained, evict-first 1.374
-        p.w_policy = wpol;
-    }
     if (w_layout == TRI_W_NK) {
-        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, bn_box, CU_TENSOR_MAP_SWIZZLE_128B);
+        st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, GM_BN, CU_TENSOR_MAP_SWIZZLE_128B);
         p.b_mn_major = 0;
         p.b_lbo = 16; p.b_sbo = 1024; p.b_kstep = 32;     // 8-row groups 1024 B apart; 16 k-values = 32 B
     } else {
-        st = make_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, 64, GM_BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, 64, GM_BK, CU_TENSOR_MAP_SWIZZLE_128B);
         p.b_mn_major = 1;
         // MN-major, 128-byte swizzle: a 64(n) x 64(k) box is 64 k-rows of 128 B (8 KiB); 8-k groups are
         // 1024 B apart (stride), the next 64 columns of n start 8192 B later (leading); 16 k-values = 2048 B.
         p.b_lbo = 8192; p.b_sbo = 1024; p.b_kstep = 2048;
     }
     if (st != TRI_OK) return st;
-    if (!one_sm) return launch_gemm_2sm(amap, wmap, p, di->sm_count, static_cast<cudaStream_t>(stream));
-
-    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
-    if (attr_gen != device_generation()) {
-        TRI_CUDA(cudaFuncSetAttribute(gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_BYTES));
-        attr_gen = device_generation();
-    }
-    const int ntiles = p.tiles_m * p.tiles_n;
-    const int grid = ntiles < di->sm_count ? ntiles : di->sm_count;
-    gemm_kernel<<<grid, GM_THREADS, GM_SMEM_BYTES, static_cast<cudaStream_t>(stream)>>>(amap, wmap, p);
-    TRI_CUDA(cudaGetLastError());
-    return TRI_OK;
+    return one_sm ? launch_gemm_1sm(amap, wmap, p, di->sm_count, s) : launch_gemm_2sm(amap, wmap, p, di->sm_count, s);
 }
 
 }  // namespace tri

@@ -17,8 +17,18 @@
 //                           CTA, so the epilogue of tile t overlaps the main loop of tile t + 1
 //   warps 4-7 epilogue      tcgen05.ld of the CTA's own 128 rows -> bf16 RNE -> swizzled shared-memory boxes -> TMA
 //                           stores (32 rows x 64 columns each); arrive on the LEADER's "tmem_empty" (8 arrivals)
-// 4096 x 18944 gives 16 x 74 = 1184 pair tiles = 74 TPCs x 16: no wave quantisation.  M index fastest, as in the
-// single-CTA kernel.  Ragged M / N / K: TMA zero fill on loads, TMA clipping on stores (the last n % 8 columns are stored from registers).
+// 4096 x 18944 gives 16 x 74 = 1184 pair tiles = 74 TPCs x 16: no wave quantisation.  M index fastest inside row-block
+// groups (tile_coords).  Ragged M / N / K: TMA zero fill on loads, TMA clipping on stores (the last n % 8 columns are
+// stored from registers).
+//
+// Tail split (gemm_common.cuh next_work): when the tile count is not a multiple of the 74 pairs, the leftover tiles of
+// the last round are cut along K into `parts` = 74 / leftover ranges, one per pair, all aligned in time like the whole
+// rounds before them (so the L2 reuse of A and W panels across pairs is untouched, which a general stream-K schedule
+// would lose).  Each pair writes its fp32 partial tile to a workspace slot of its own; splitk_reduce_kernel, launched
+// behind this kernel with programmatic stream serialization, adds the parts in a fixed order (deterministic), rounds to
+// bf16 and stores.  (Adding the partials with red.global.add.v4.f32 instead was measured: 1.2 M contended vector atomics
+// on two tiles cost ~45 us.)  Down-projection 4096 x 3584 x 18944: 224 tiles = 3 rounds + 2 tiles x 37 parts of 8
+// k-blocks instead of a fourth round.
 #include "tri_internal.h"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
@@ -35,17 +45,6 @@ constexpr int G2_THREADS = 256;
 constexpr int G2_TMEM_COLS = 512;
 constexpr int G2_OUT_BYTES = 4 * 2 * 4096;                 // epilogue staging: per warp two 32-row x 64-column bf16 boxes
 constexpr int G2_SMEM_BYTES = 1024 + G2_STAGES * G2_STAGE_BYTES + G2_OUT_BYTES + 256;
-
-// Tile order: M index fastest inside groups of p.group_m row blocks, groups one after the other.  A group's A panels
-// (group_m x 256 rows x K) stay L2-resident while the W panels stream past once per group; group_m = all row blocks
-// when A fits (config 4: 29 MB), smaller for tall A so that the resident set stays near 32 MB.
-__device__ __forceinline__ void tile_coords(const GemmParams &p, int t, int &tm, int &tn)
-{
-    const int per_group = p.group_m * p.tiles_n, grp = t / per_group, r = t - grp * per_group;
-    const int m0 = grp * p.group_m, gm = (p.tiles_m - m0 < p.group_m) ? p.tiles_m - m0 : p.group_m;
-    tm = m0 + r % gm;
-    tn = r / gm;
-}
 
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(G2_THREADS, 1)
 gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap,
@@ -65,6 +64,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
     const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
     const int ntiles = p.tiles_m * p.tiles_n;             // pair tiles (tiles_m counts 256-row blocks)
 
+    if (p.parts > 1) ptx::pdl_launch_dependents();        // splitk_reduce_kernel may take its place; it waits for this grid
     if (threadIdx.x == 0) {
         for (int s = 0; s < G2_STAGES; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);             // leader's copy is the one used
@@ -94,14 +94,15 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
             // a W panel is read by the 16 pairs that share its tn within one wave: it must survive in L2 until the last of
             // them has passed (evict-first lets it go early: 304 MB of DRAM reads per call instead of the 165 MB of A + W);
             // measured on config 4, sustained: evict-first 1.374, evict-normal 1.371, evict-last 1.392 PFLOP/s
-            const uint64_t pol_w = (p.w_policy == 0) ? ptx::policy_evict_first() : (p.w_policy == 1) ? ptx::policy_evict_normal() : ptx::policy_evict_last();
+            const uint64_t pol_w = ptx::policy_evict_last();
             const uint64_t pol_a = ptx::policy_evict_last();
             uint32_t it = 0;
-            for (int t = pair; t < ntiles; t += npairs) {
+            GemmWork wk;
+            for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i) {
                 int tm, tn;
-            tile_coords(p, t, tm, tn);
+                tile_coords(p, wk.tile, tm, tn);
                 const int row0 = tm * (2 * G2_BM) + (int)rank * G2_BM, col0 = tn * G2_BN + (int)rank * G2_BNH;
-                for (int kb = 0; kb < p.kblocks; ++kb, ++it) {
+                for (int kb = wk.kb0; kb < wk.kb1; ++kb, ++it) {
                     const uint32_t s = it % G2_STAGES, ph = (it / G2_STAGES) & 1;
                     ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);
                     const uint32_t fb = full0 + 8 * s;
@@ -123,12 +124,13 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         if (ptx::elect_one()) {
             const uint32_t idesc = make_idesc(2 * G2_BM, G2_BN, p.b_mn_major);
             uint32_t it = 0, tcount = 0;
-            for (int t = pair; t < ntiles; t += npairs, ++tcount) {
+            GemmWork wk;
+            for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i, ++tcount) {
                 const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
                 ptx::mbar_wait(tempty0 + 8 * acc, aph ^ 1);          // both epilogues have drained this accumulator
                 ptx::tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * G2_BN;
-                for (int kb = 0; kb < p.kblocks; ++kb, ++it) {
+                for (int kb = wk.kb0; kb < wk.kb1; ++kb, ++it) {
                     const uint32_t s = it % G2_STAGES, ph = (it / G2_STAGES) & 1;
                     ptx::mbar_wait(full0 + 8 * s, ph);
                     ptx::tc_fence_after();
@@ -138,7 +140,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
 #pragma unroll
                     for (int kk = 0; kk < G2_BK / 16; ++kk)
                         ptx::mma_bf16_ss_2sm(d_tmem, adesc + (uint64_t)((kk * 32) >> 4), bdesc + (uint64_t)((kk * p.b_kstep) >> 4),
-                                             idesc, (kb | kk) != 0);
+                                             idesc, (kb > wk.kb0) | (kk != 0));
                     ptx::mma_commit_2sm(empty0 + 8 * s);             // stage free in both CTAs once these MMAs retire
                 }
                 ptx::mma_commit_2sm(tfull0 + 8 * acc);               // accumulators complete in both CTAs
@@ -155,14 +157,30 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         const uint32_t stage0 = outbuf + ew * 8192;
         uint32_t tcount = 0, sb = 0;
         if (lane == 0) ptx::prefetch_tmap(&cmap);
-        for (int t = pair; t < ntiles; t += npairs, ++tcount) {
+        GemmWork wk;
+        for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i, ++tcount) {
             int tm, tn;
-            tile_coords(p, t, tm, tn);
+            tile_coords(p, wk.tile, tm, tn);
             const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
             ptx::mbar_wait(tfull0 + 8 * acc, aph);
             ptx::tc_fence_after();
             const int row0 = tm * (2 * G2_BM) + (int)rank * G2_BM + ew * 32;
             const uint32_t taddr = tmem_base + acc * G2_BN + ((uint32_t)(ew * 32) << 16);
+            if (wk.split >= 0) {
+                // split tile: this warp's 32 x 256 slice of the pair's partial sums goes to the workspace, nothing to C
+                float *slice = p.ws + ((size_t)(wk.split * p.parts + wk.part) * 8 + (size_t)rank * 4 + ew) * (32 * G2_BN);
+#pragma unroll 1
+                for (int blk = 0; blk < G2_BN / 32; ++blk) {
+                    uint32_t r[32];
+                    ptx::tmem_ld_32x32b_x32(taddr + blk * 32, r);
+                    ptx::tmem_ld_wait();
+                    splitk_put(slice, blk, lane, r);
+                }
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_cluster(tempty0 + 8 * acc, 0);
+                continue;
+            }
 #pragma unroll 1
             for (int g = 0; g < G2_BN / 64; ++g, sb ^= 1) {
                 const uint32_t buf = stage0 + sb * 4096;
@@ -201,8 +219,10 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
                 }
                 ptx::fence_proxy_async_smem();                        // generic-proxy writes visible to the TMA engine
                 __syncwarp();
-                if (lane == 0 && row0 < p.m && tn * G2_BN + g * 64 < (p.n & ~7)) {
-                    ptx::tma_store_2d(&cmap, buf, tn * G2_BN + g * 64, row0);
+                if (lane == 0) {
+                    if (row0 < p.m && tn * G2_BN + g * 64 < (p.n & ~7)) ptx::tma_store_2d(&cmap, buf, tn * G2_BN + g * 64, row0);
+                    // one bulk group per buffer toggle, also when nothing was stored (an empty group is legal): wait_read<1>
+                    // above counts groups, and must mean "the store before the previous one" for the buffer it guards
                     ptx::tma_store_commit();
                 }
             }
@@ -224,15 +244,14 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
 {
     CUtensorMap cmap;     // C as 64-column x 32-row boxes for the epilogue's TMA stores (out-of-range rows / columns are clipped)
     const int n8 = p.n & ~7;     // see the epilogue: the last n % 8 columns do not go through TMA
-    int st = make_tmap_2d_bf16(&cmap, p.c, (uint64_t)(n8 ? n8 : 8), (uint64_t)p.m, (uint64_t)p.ldc * 2, 64, 32, CU_TENSOR_MAP_SWIZZLE_128B);
+    int st = cached_tmap_2d_bf16(&cmap, p.c, (uint64_t)(n8 ? n8 : 8), (uint64_t)p.m, (uint64_t)p.ldc * 2, 64, 32, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
     static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
     if (attr_gen != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_2sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES));
         attr_gen = device_generation();
     }
-    const int ntiles = p.tiles_m * p.tiles_n;
-    const int pairs = ntiles < sm_count / 2 ? ntiles : sm_count / 2;
+    const int ntiles = p.tiles_m * p.tiles_n, max_pairs = sm_count / 2;
     GemmParams q = p;
     {   // rows of A kept resident: about 32 MB worth of 256-row panels, at least 4, all of them when A is small
         const double panel = 256.0 * p.k * 2.0;
@@ -240,8 +259,26 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
         g = g < 4 ? 4 : g;
         q.group_m = g < p.tiles_m ? g : p.tiles_m;
     }
+    // Tail split: the leftover tiles of the last round, each cut into `parts` k-ranges (one per pair).  Worth it when the
+    // time saved, (1 - 1/parts) of a tile = of kblocks k-blocks, clearly exceeds the fixed cost of writing a 256 x 256 fp32
+    // partial per pair and the reduction kernel behind (a few microseconds = a few k-blocks' worth).
+    const int left = ntiles % max_pairs;
+    int parts = left ? max_pairs / left : 1;
+    if (parts > p.kblocks / 8) parts = p.kblocks / 8;             // at least 8 k-blocks per part (4096 x 3584 x 3584: 7 parts 72 us, 37 parts 76 us, none 78 us)
+    q.full_tiles = ntiles;
+    q.parts = 1;
+    q.ws = nullptr;
+    int pairs = ntiles < max_pairs ? ntiles : max_pairs;
+    if (parts >= 2 && (parts - 1) * p.kblocks >= 24 * parts) {
+        q.full_tiles = ntiles - left;
+        q.parts = parts;
+        st = splitk_workspace(s, (size_t)left * parts * (2 * G2_BM) * G2_BN * sizeof(float), &q.ws);
+        if (st != TRI_OK) return st;
+        if (q.full_tiles == 0) pairs = left * parts;
+    }
     gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, cmap, q);
     TRI_CUDA(cudaGetLastError());
+    if (q.parts > 1) return launch_splitk_reduce(q, 2 * G2_BM, G2_BN, true, s);
     return TRI_OK;
 }
 

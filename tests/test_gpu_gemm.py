@@ -131,3 +131,73 @@ def test_config4_sampled_rows(layout):
     got = dc.view(torch.bfloat16)[::97].float()
     assert torch.isfinite(got).all()
     assert (got - ref).abs().max().item() < 0.08
+
+
+def _gemm_twice(a, wp, m, n, k, layout):
+    """Two calls into the same output: the second one must find the split-K workspace and counters clean."""
+    c1 = run_gemm(a, wp, m, n, k, layout)
+    c2 = run_gemm(a, wp, m, n, k, layout)
+    assert (c1 == c2).all(), "second call differs: split-K workspace not restored"
+    return c2
+
+
+@pytest.mark.parametrize("layout", LAYOUTS)
+@pytest.mark.parametrize("m,n,k", [(300, 704, 2048),      # 6 pair tiles < 74 pairs: every tile cut 12 ways
+                                   (256, 19456, 1664),    # 76 pair tiles: one round + 2 tiles cut 26 ways (one k-block each)
+                                   (520, 6504, 1664)])    # 3 x 26 = 78 tiles: one round + 4 tiles cut 18 ways, ragged M, N and k-ranges
+def test_pair_kernel_tail_split(layout, m, n, k):
+    """The tail split of the CTA-pair kernel (gemm_common.cuh next_work, splitk_*): fp32 partial tiles added through L2,
+    last arriver stores; checked on stratified rows against the oracle, called twice."""
+    a = normal_bf16(90, (m, k))
+    w = normal_bf16(91, (k, n), 0.05)
+    wp = phys_w(w, layout)
+    c = _gemm_twice(a, wp, m, n, k, layout)
+    rows = stratified_rows(90, m, min(m, 40))
+    check_rows(c[rows], a, wp, layout, rows=rows)
+
+
+@pytest.mark.parametrize("layout", LAYOUTS)
+def test_down_projection_sampled_rows(layout):
+    """Thinker MLP down-projection at prefill size: 4096 x 3584 x 18944, 224 pair tiles = 3 rounds + 2 tiles
+    cut 37 ways; 64 stratified rows x all 3584 columns, stated bound; no NaN filler left anywhere."""
+    m, k, n = 4096, 18944, 3584
+    a = normal_bf16(5, (m, k), 1.0, stream=0)
+    w = normal_bf16(5, (k, n), 0.02, stream=1)
+    wp = phys_w(w, layout)
+    da, dw = to_dev(a), to_dev(wp)
+    dc = torch.full((m, n), 0x7FC0, dtype=torch.int16, device="cuda")
+    for _ in range(2):
+        tri.prefill_gemm(m, n, k, da, k, dw, wp.shape[1], layout, dc, n)
+    torch.cuda.synchronize()
+    rows = stratified_rows(5, m, 64)
+    c_rows = dc[torch.from_numpy(rows.astype(np.int64)).cuda()].cpu().numpy().view(np.uint16)
+    check_rows(c_rows, a, wp, layout, rows=rows, stated=True)
+    assert torch.isfinite(dc.view(torch.bfloat16).float()).all()
+
+
+@pytest.mark.parametrize("layout", LAYOUTS)
+@pytest.mark.parametrize("m", [16, 64, 128])
+def test_short_a_up_projection(layout, m):
+    """m <= 128 runs the one-CTA kernel (128 x 128 tiles): the config-4 weights with a short A; 148 tiles, no split."""
+    k, n = 3584, 18944
+    a = normal_bf16(3, (m, k), 1.0, stream=4)
+    w = normal_bf16(3, (k, n), 0.02, stream=1)
+    wp = phys_w(w, layout)
+    c = run_gemm(a, wp, m, n, k, layout)
+    rows = stratified_rows(6, m, min(m, 24))
+    check_rows(c[rows], a, wp, layout, rows=rows, stated=True)
+    assert np.isfinite(bf16_bits_to_f32(c)).all()
+
+
+@pytest.mark.parametrize("layout", LAYOUTS)
+@pytest.mark.parametrize("m,n,k", [(64, 3584, 18944),     # down-projection, 28 tiles cut 5 ways (59-60 k-blocks each)
+                                   (100, 304, 1024),      # 3 tiles cut 16 ways, one k-block each
+                                   (17, 136, 4104),       # ragged last k-block, 2 tiles cut 65 ways
+                                   (128, 19000, 640)])    # 149 tiles: one round + 1 tile cut 10 ways
+def test_one_cta_kernel_split_k(layout, m, n, k):
+    a = normal_bf16(92, (m, k))
+    w = normal_bf16(93, (k, n), 0.03)
+    wp = phys_w(w, layout)
+    c = _gemm_twice(a, wp, m, n, k, layout)
+    rows = stratified_rows(92, m, min(m, 16))
+    check_rows(c[rows], a, wp, layout, rows=rows)
