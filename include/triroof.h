@@ -229,13 +229,19 @@ double tri_model_phi(const tri_model *m, double ai, double f_mhz);
 double tri_model_power(const tri_model *m, double ai, int32_t i);
 /* Eq. 5: duration-weighted A.I. of a phase, sum(d_i ai_i) / sum(d_i); NaN if n == 0 or sum(d) <= 0. */
 double tri_phase_ai(const double *d, const double *ai, size_t n);
+/* The premise of the Eq. 6 solver, checked ONCE per (model, phase A.I.) — O(n_f): the clock table is positive and
+ * strictly ascending, the power tables non-negative, p_tdp positive, and at this A.I. theta(ai, f) and the modelled
+ * power are non-decreasing along the table ("monotone frequency levels").  TRI_ERR_INVALID_ARG otherwise. */
+int tri_model_validate(const tri_model *m, double ai);
 /* Eq. 6: among the supported clocks f <= f_limit_mhz with theta(ai, f) >= (1 - eps) * theta(ai, f_max)
  * (f_max = the highest supported clock), the one of least modelled power; ties go to the HIGHEST such clock
- * ("the highest frequency that achieves this lower power").  Solved as the paper does, by binary search over
- * the discrete levels, which is exact when theta is non-decreasing in f and the modelled power is
- * non-decreasing in f up to the cap; TRI_ERR_INVALID_ARG if the tables violate that (checked), or
- * if eps is outside [0, 1), or no clock <= f_limit_mhz exists.  If no clock meets the throughput constraint the
- * highest clock <= f_limit_mhz is returned (best effort, *feasible = 0).  Outputs: index into f_mhz, and flag. */
+ * ("the highest frequency that achieves this lower power").  Solved as the paper does — "a low-overhead solver ...
+ * for every decode period", P:186-188 — by three binary searches over the discrete levels: O(log n_f) model
+ * evaluations, no scan of the tables.  Exact on a model that passed tri_model_validate(m, ai); on one that would not,
+ * the result is still an index <= the highest clock <= f_limit_mhz, but need not be the optimum.
+ * TRI_ERR_INVALID_ARG if a pointer is NULL, n_f < 1, ai / f_limit_mhz is not positive, eps is outside [0, 1), or no
+ * clock <= f_limit_mhz exists.  If no clock meets the throughput constraint the highest clock <= f_limit_mhz is
+ * returned (best effort, *feasible = 0).  Outputs: index into f_mhz, and flag. */
 int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double eps, int32_t *index, int32_t *feasible);
 /* Fit of Eq. 4 to n measured points (ai_i, f_i, theta_i) at a caller-chosen gamma: beta = mean of theta / ai over
  * the points with ai <= ai_mem (memory branch); on the compute branch f / theta = 1 / eta + (omega / eta) * f^gamma / ai

@@ -39,7 +39,7 @@ B_DEFAULT = 0.0009765625
 EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "tri_sm_count", "tri_l2_bytes",
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
-           "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_solve_clock",
+           "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_model_validate", "tri_solve_clock",
            "tri_fit_theta", "tri_fit_power", "tri_probe_fma_issue"]
 
 
@@ -125,6 +125,7 @@ def lib():
     L.tri_model_power.restype = c_double
     L.tri_phase_ai.argtypes = [POINTER(c_double), POINTER(c_double), c_size_t]
     L.tri_phase_ai.restype = c_double
+    L.tri_model_validate.argtypes = [POINTER(tri_model), c_double]
     L.tri_solve_clock.argtypes = [POINTER(tri_model), c_double, c_double, c_double, POINTER(c_int32), POINTER(c_int32)]
     L.tri_fit_theta.argtypes = [POINTER(c_double), POINTER(c_double), POINTER(c_double), c_size_t, c_double, c_double, c_double,
                                 POINTER(tri_model)]
@@ -309,6 +310,10 @@ class Model:
     def power(self, ai, i):
         return lib().tri_model_power(byref(self.c), ai, i)
 
+    def validate(self, ai):
+        """The premise of solve_clock at this A.I. (tables well formed, theta and power monotone in f); raises TriError."""
+        _check(lib().tri_model_validate(byref(self.c), ai), "tri_model_validate")
+
     def solve_clock(self, ai, f_limit_mhz, eps):
         """Eq. 6 -> (index into f_mhz, feasible)."""
         idx, feas = c_int32(-1), c_int32(0)
@@ -358,6 +363,10 @@ def tri_model_phi(model: Model, ai: float, f_mhz: float) -> float:
 
 def tri_model_power(model: Model, ai: float, i: int) -> float:
     return model.power(ai, i)
+
+
+def tri_model_validate(model: Model, ai: float) -> None:
+    model.validate(ai)
 
 
 def tri_solve_clock(model: Model, ai: float, f_limit_mhz: float, eps: float):

@@ -77,10 +77,28 @@ double tri_phase_ai(const double *d, const double *ai, size_t n)
     return den > 0.0 ? num / den : NAN;
 }
 
-int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double eps, int32_t *index, int32_t *feasible)
+int tri_model_validate(const tri_model *m, double ai)
 {
     int st = tri::check_model(m, true);
     if (st != TRI_OK) return st;
+    if (!tri::pos(ai)) return tri::fail(TRI_ERR_INVALID_ARG, "ai must be positive");
+    // the premise of the binary search (P:186-188): throughput and modelled power do not decrease with the clock
+    for (int i = 1; i < m->n_f; ++i) {
+        if (tri::theta(m, ai, m->f_mhz[i]) < tri::theta(m, ai, m->f_mhz[i - 1]) * (1.0 - 1e-12) ||
+            tri::power(m, ai, i) < tri::power(m, ai, i - 1) * (1.0 - 1e-12))
+            return tri::fail(TRI_ERR_INVALID_ARG, "model is not monotone in f at A.I. %g (clock %g MHz): binary search does not apply", ai,
+                             m->f_mhz[i]);
+    }
+    return TRI_OK;
+}
+
+int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double eps, int32_t *index, int32_t *feasible)
+{
+    // O(1) checks only: the tables are validated once by tri_model_validate, not per decode period
+    int st = tri::check_model(m, false);
+    if (st != TRI_OK) return st;
+    if (m->n_f < 1 || !m->f_mhz || !m->p_idle_w || !m->p_dyn_w || !tri::pos(m->p_tdp))
+        return tri::fail(TRI_ERR_INVALID_ARG, "clock / power tables missing or p_tdp not positive");
     if (!index || !feasible) return tri::fail(TRI_ERR_INVALID_ARG, "index / feasible is NULL");
     if (!tri::pos(ai) || !tri::pos(f_limit_mhz) || !(eps >= 0.0 && eps < 1.0))
         return tri::fail(TRI_ERR_INVALID_ARG, "ai, f_limit must be positive, eps in [0, 1)");
@@ -92,13 +110,6 @@ int tri_solve_clock(const tri_model *m, double ai, double f_limit_mhz, double ep
         if (m->f_mhz[mid] <= f_limit_mhz) lo = mid; else hi = mid - 1;
     }
     const int top = lo;
-    // the premise of the binary search (P:186-188): throughput and modelled power do not decrease with the clock
-    for (int i = 1; i < m->n_f; ++i) {
-        if (tri::theta(m, ai, m->f_mhz[i]) < tri::theta(m, ai, m->f_mhz[i - 1]) * (1.0 - 1e-12) ||
-            tri::power(m, ai, i) < tri::power(m, ai, i - 1) * (1.0 - 1e-12))
-            return tri::fail(TRI_ERR_INVALID_ARG, "model is not monotone in f at A.I. %g (clock %g MHz): binary search does not apply", ai,
-                             m->f_mhz[i]);
-    }
     const double need = (1.0 - eps) * tri::theta(m, ai, m->f_mhz[m->n_f - 1]);
     if (tri::theta(m, ai, m->f_mhz[top]) < need) {           // even the highest allowed clock is too slow
         *index = top;

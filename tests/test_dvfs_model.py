@@ -55,14 +55,18 @@ def test_solver_binary_search_equals_exhaustive_search():
         f_limit = float(rng.choice([kw["f_mhz"][-1], rng.uniform(kw["f_mhz"][0], kw["f_mhz"][-1] + 50.0)]))
         eps = float(rng.choice([0.0, 0.02, 0.05, 0.2, rng.uniform(0.0, 0.9)]))
         try:
-            got = m.solve_clock(ai, f_limit, eps)
+            m.validate(ai)                              # once per (model, A.I.): the solver itself does no table scan
         except tri.TriError as e:                       # the library refuses tables on which the binary search is not exact
             assert e.status == tri.TRI_ERR_INVALID_ARG
             f, th = kw["f_mhz"], [o.theta(ai, x, kw["eta"], kw["beta"], kw["omega"], kw["gamma"]) for x in kw["f_mhz"]]
             pw = [o.power(ai, x, kw["p_idle_w"][i], kw["p_dyn_w"][i], kw["p_tdp"], kw["eta"], kw["beta"]) for i, x in enumerate(f)]
             assert any(b < a for a, b in zip(th, th[1:])) or any(b < a for a, b in zip(pw, pw[1:]))
             rejected += 1
+            top = max(i for i, x in enumerate(f) if x <= f_limit)
+            idx, _ = m.solve_clock(ai, f_limit, eps)    # unvalidated tables: still a legal index, not necessarily the optimum
+            assert 0 <= idx <= top
             continue
+        got = m.solve_clock(ai, f_limit, eps)
         want = o.solve_clock(ai, kw["f_mhz"], kw["p_idle_w"], kw["p_dyn_w"], kw["p_tdp"], kw["eta"], kw["beta"], kw["omega"],
                              kw["gamma"], f_limit, eps)
         assert got == want, (kw, ai, f_limit, eps)
@@ -76,9 +80,36 @@ def test_solver_argument_errors():
     for bad in [(-1.0, 2000.0, 0.05), (1.0, 2000.0, 1.0), (1.0, 2000.0, -0.1), (1.0, kw["f_mhz"][0] - 1.0, 0.05)]:
         with pytest.raises(tri.TriError):
             m.solve_clock(*bad)
-    kw["f_mhz"][3] = kw["f_mhz"][2]                     # not strictly ascending
+    kw["f_mhz"][3] = kw["f_mhz"][2]                     # not strictly ascending: the validator's business
     with pytest.raises(tri.TriError):
-        tri.Model(**kw).solve_clock(1.0, 5000.0, 0.05)
+        tri.Model(**kw).validate(1.0)
+
+
+def test_solver_is_logarithmic_in_the_table_size():
+    """"a low-overhead solver ... for every decode period".  tri_solve_clock evaluates the model O(log n_f)
+    times and never scans the tables: its time on a 2^20-entry table is within a small factor of a 2^6-entry one, while
+    the one-time tri_model_validate grows with n_f."""
+    import time
+
+    def model(n):
+        f = np.linspace(200.0, 2000.0, n)
+        return tri.Model(0.0379, 6.54, 0.02, 0.5, 1e9, list(f), list(60.0 + 0.05 * f), list(2e-4 * f * f))
+
+    def per_call(fn, reps):
+        fn()
+        t = time.perf_counter()
+        for _ in range(reps):
+            fn()
+        return (time.perf_counter() - t) / reps
+
+    small, big = model(1 << 6), model(1 << 20)
+    big.validate(100.0)
+    assert small.solve_clock(100.0, 2000.0, 0.05)[1] and big.solve_clock(100.0, 2000.0, 0.05)[1]
+    t_small = per_call(lambda: small.solve_clock(100.0, 2000.0, 0.05), 2000)
+    t_big = per_call(lambda: big.solve_clock(100.0, 2000.0, 0.05), 2000)
+    t_val = per_call(lambda: big.validate(100.0), 3)
+    assert t_big < 8 * t_small + 20e-6, (t_small, t_big)          # 20 vs 6 bisection levels plus the ctypes call
+    assert t_val > 50 * t_big, (t_val, t_big)                       # the scan is what was moved out of the solver
 
 
 def test_fit_matches_oracle_on_noisy_sweep():

@@ -93,3 +93,30 @@ def test_fit_recovers_planted_parameters():
     got = o.fit_theta(ai, f, th, ai_mem=2, ai_cmp=64, gamma=gamma)
     assert got["eta"] == pytest.approx(eta, rel=1e-6) and got["beta"] == pytest.approx(beta, rel=1e-12)
     assert got["omega"] == pytest.approx(omega, rel=1e-5)
+
+
+def test_fit_power_recovers_a_planted_line():
+    """Pin of oracle.fit_power on its own (not against the product): Eq. 2 at one clock is P = P_idle + P_dyn * phi, so
+    points planted on that line at the selected clock come back as (P_idle, P_dyn) exactly; points at other clocks and
+    points at / above the cap must not enter the fit (above the cap the measured power says nothing about
+    P_dyn)."""
+    eta, beta = 0.0379, 6.54
+    p_idle, p_dyn, cap = 480.0, 770.0, 1000.0
+    ai = np.array([0.25, 1, 4, 8, 16, 24, 32, 50, 64, 100, 128, 200, 256, 512, 1024], float)
+    f = np.where(ai < 8, 1700.0, 1965.0)                                    # two clock columns; A.I. 8 and 16 at 1965 MHz sit at the cap
+    p = np.array([min(p_idle + p_dyn * o.phi(a, x, eta, beta), cap) for a, x in zip(ai, f)])
+    got = o.fit_power(ai, f, p, eta, beta, 1965.0, 1.0, cap - 10.0)
+    below = int(((f == 1965.0) & (p < cap - 10.0)).sum())
+    assert got["n_used"] == below and 2 <= below < int((f == 1965.0).sum())         # the capped points were dropped
+    assert got["p_idle_w"] == pytest.approx(p_idle, rel=1e-9) and got["p_dyn_w"] == pytest.approx(p_dyn, rel=1e-9)
+    # the other clock column has its own line: a different planted pair is recovered from the same call on that column
+    p2 = np.where(f == 1700.0, 300.0 + 500.0 * np.array([o.phi(a, x, eta, beta) for a, x in zip(ai, f)]), p)
+    got2 = o.fit_power(ai, f, p2, eta, beta, 1700.0, 1.0, cap)
+    assert got2["n_used"] == int((f == 1700.0).sum())
+    assert got2["p_idle_w"] == pytest.approx(300.0, rel=1e-9) and got2["p_dyn_w"] == pytest.approx(500.0, rel=1e-9)
+    # a dropped intercept or swapped regressors would fail: slope and intercept are distinct and both non-zero
+    assert abs(got["p_idle_w"] - got["p_dyn_w"]) > 100.0
+    # two points fix the line: hand-worked, phi = 0.5 -> 865 W, phi = 0.25 -> 672.5 W at P_idle 480, P_dyn 770
+    a1, a2 = eta * 1965.0 / beta / 0.5, eta * 1965.0 / beta / 0.25          # compute-bound side: phi = eta f / (beta ai)
+    g = o.fit_power([a1, a2], [1965.0, 1965.0], [865.0, 672.5], eta, beta, 1965.0, 0.0, cap)
+    assert g["p_idle_w"] == pytest.approx(480.0, rel=1e-9) and g["p_dyn_w"] == pytest.approx(770.0, rel=1e-9)
