@@ -37,6 +37,7 @@ struct GemmParams {
     // order, by splitk_reduce_kernel.
     int full_tiles, parts;
     int a_box_bytes;         // bytes of one A box (one-CTA kernel: the box holds only the rows that exist)
+    int stages;              // one-CTA kernel: ring depth
     float *ws;               // fp32 workspace: [split tile][part][warp slice][fragment order]
 };
 

@@ -8,7 +8,7 @@
 // One-CTA kernel (m <= 128: chunked-prefill tails, speculative / large-batch decode): weight-streaming bound, so the
 // tile is 128 x 128 — 148 tiles for n = 18944, one per SM — and when there are fewer tiles than SMs every tile is cut
 // along K into `parts` ranges (gemm_common.cuh next_work / splitk_*) so that all SMs pull on HBM.  Warp roles as in the
-// pair kernel: warp 0 TMA producer (A 128 x 64 and W 128 x 64 per k-block into a 6-stage ring, 128-byte swizzle), warp 1
+// pair kernel: warp 0 TMA producer (A rows x 64 and W 128 x 64 per k-block into a 6- to 12-stage ring, 128-byte swizzle), warp 1
 // MMA issuer (tcgen05.mma.cta_group::1.kind::f16, M 128, N 128, K 16), warp 2 TMEM owner (two 128-column accumulators),
 // warps 4-7 epilogue (tcgen05.ld -> cvt.rn.bf16x2 -> 16-byte global stores; the output is small here).
 // Ragged M / N / K: TMA zero-fills out-of-bounds reads; stores clip.
@@ -25,24 +25,26 @@
 namespace tri {
 
 constexpr int GM_BM = 128, GM_BN = 128, GM_BK = 64;
-constexpr int GM_STAGES = 6;
-constexpr int GM_A_BYTES = GM_BM * GM_BK * 2;      // 16 KiB
+constexpr int GM_MAX_STAGES = 12;                  // ring depth is chosen per call: the A box shrinks with m, the ring grows
 constexpr int GM_B_BYTES = GM_BN * GM_BK * 2;      // 16 KiB
-constexpr int GM_STAGE_BYTES = GM_A_BYTES + GM_B_BYTES;
 constexpr int GM_THREADS = 256;
 constexpr int GM_TMEM_COLS = 2 * GM_BN;
-constexpr int GM_SMEM_BYTES = 1024 + GM_STAGES * GM_STAGE_BYTES + 256;
+constexpr int GM_BAR_BYTES = 16 * GM_MAX_STAGES + 64;
+constexpr int GM_SMEM_MAX = 220 * 1024;
+
+__host__ __device__ constexpr int gm_smem_bytes(int stages, int stage_bytes) { return 1024 + stages * stage_bytes + GM_BAR_BYTES; }
 
 __global__ void __launch_bounds__(GM_THREADS, 1)
 gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap wmap, const GemmParams p)
 {
     extern __shared__ uint8_t smem_raw[];
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int GM_STAGES = p.stages, GM_STAGE_BYTES = p.a_box_bytes + GM_B_BYTES, GM_A_BYTES = p.a_box_bytes;   // per call (see gemm_impl)
     const uint32_t ring = ptx::smem_u32(smem);
     const uint32_t bars = ring + GM_STAGES * GM_STAGE_BYTES;
-    const uint32_t full0 = bars, empty0 = bars + 8 * GM_STAGES;
-    const uint32_t tfull0 = bars + 16 * GM_STAGES, tempty0 = tfull0 + 16;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + GM_STAGES * GM_STAGE_BYTES + 16 * GM_STAGES + 32);
+    const uint32_t full0 = bars, empty0 = bars + 8 * GM_MAX_STAGES;
+    const uint32_t tfull0 = bars + 16 * GM_MAX_STAGES, tempty0 = tfull0 + 16;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + GM_STAGES * GM_STAGE_BYTES + 16 * GM_MAX_STAGES + 32);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ntiles = p.tiles_m * p.tiles_n, me = blockIdx.x, nw = gridDim.x;
@@ -83,7 +85,7 @@ gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
                     const uint32_t s = it % GM_STAGES, ph = (it / GM_STAGES) & 1;
                     ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);
                     const uint32_t fb = full0 + 8 * s;
-                    ptx::mbar_arrive_expect_tx(fb, p.a_box_bytes + GM_B_BYTES);
+                    ptx::mbar_arrive_expect_tx(fb, GM_STAGE_BYTES);
                     const uint32_t sa = ring + s * GM_STAGE_BYTES, sb = sa + GM_A_BYTES;
                     ptx::tma_load_2d_hint(sa, &amap, kb * GM_BK, tm * GM_BM, fb, pol_a);
                     if (!p.b_mn_major) {
@@ -304,10 +306,16 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
 {
     static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
     if (attr_gen != device_generation()) {
-        TRI_CUDA(cudaFuncSetAttribute(gemm_1sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_BYTES));
+        TRI_CUDA(cudaFuncSetAttribute(gemm_1sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_MAX));
         attr_gen = device_generation();
     }
     GemmParams q = p;
+    // Ring depth: as many stages as fit (a stage is the A box + 16 KiB of W).  The kernel is bound by the weight stream,
+    // and what keeps HBM busy is bytes in flight per SM: 6 stages (m = 128) .. 12 stages (m <= 16: 192 KiB of W in flight).
+    const int stage_bytes = p.a_box_bytes + GM_B_BYTES;
+    q.stages = (GM_SMEM_MAX - 1024 - GM_BAR_BYTES) / stage_bytes;
+    if (q.stages > GM_MAX_STAGES) q.stages = GM_MAX_STAGES;
+    const int smem_bytes = gm_smem_bytes(q.stages, stage_bytes);
     const int ntiles = p.tiles_m * p.tiles_n;
     const int left = ntiles % sm_count;
     int parts = left ? sm_count / left : 1;
@@ -323,7 +331,7 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
         if (st != TRI_OK) return st;
         if (q.full_tiles == 0) grid = left * parts;
     }
-    gemm_1sm_kernel<<<grid, GM_THREADS, GM_SMEM_BYTES, s>>>(amap, wmap, q);
+    gemm_1sm_kernel<<<grid, GM_THREADS, smem_bytes, s>>>(amap, wmap, q);
     TRI_CUDA(cudaGetLastError());
     if (q.parts > 1) return launch_splitk_reduce(q, GM_BM, GM_BN, false, s);
     return TRI_OK;

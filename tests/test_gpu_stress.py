@@ -1,0 +1,94 @@
+"""Race / ordering stress of the asynchronous paths, in place of compute-sanitizer (closed on this pool: profiles/r2_sanitizer.md).
+What a race in the mbarrier / TMEM / TMA-store / split-K code would show as is run-to-run variation or a stale tile, so every
+case here runs a kernel many times back to back with no host synchronisation in between, into NaN-prefilled outputs, and
+demands that every repetition is bit-identical to the first and that the first is within the oracle's bound."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_29629_b200 as tri
+from synth_inputs import bf16_bits_to_f32, normal_bf16
+from tests.tolerance import widened_bound
+
+pytestmark = pytest.mark.gpu
+NAN16 = 0x7FC0
+
+
+def dev(bits):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda()
+
+
+def within_bound(c_bits, a, wp, layout):
+    r = oracle.gemm_rows(a, wp, w_layout=layout)
+    g = bf16_bits_to_f32(c_bits).astype(np.float64)
+    assert np.isfinite(g).all()
+    assert (np.abs(g - r["c64"]) <= widened_bound(r["c64"], r["s64"], a.shape[1])).all()
+
+
+@pytest.mark.parametrize("m,n,k", [(300, 129, 512),     # pair kernel; column groups 2, 3 of the only tile store nothing (ADVICE: bulk-group count)
+                                   (257, 136, 256),     # second row block almost empty: whole warps skip their stores
+                                   (520, 1096, 640),    # 3 x 5 tiles, ragged in both directions, two tiles per pair never happens: one round
+                                   (1536, 4352, 448),   # 204 tiles: three rounds, both accumulators, ring wrap-arounds
+                                   (300, 704, 2048),    # pair kernel, every tile cut 12 ways + reduction kernel under PDL
+                                   (64, 3584, 2048),    # one-CTA kernel, 28 tiles cut 5 ways
+                                   (100, 1000, 256)])   # one-CTA kernel, whole tiles
+def test_gemm_back_to_back_is_bit_stable(m, n, k):
+    a, w = normal_bf16(95, (m, k)), normal_bf16(96, (k, n), 0.05)
+    wp = np.ascontiguousarray(w.T)
+    da, dw = dev(a), dev(wp)
+    reps, ldc = 24, (n + 7) // 8 * 8
+    outs = [torch.full((m, ldc), NAN16, dtype=torch.int16, device="cuda") for _ in range(reps)]
+    for c in outs:                                        # no synchronisation between the calls
+        tri.prefill_gemm(m, n, k, da, k, dw, k, tri.TRI_W_NK, c, ldc)
+    torch.cuda.synchronize()
+    first = outs[0].cpu().numpy().view(np.uint16)
+    assert (first[:, n:] == NAN16).all(), "kernel wrote outside its n columns"
+    within_bound(first[:, :n], a, wp, tri.TRI_W_NK)
+    for i, c in enumerate(outs[1:], 1):
+        assert torch.equal(c, outs[0]), f"repetition {i} differs from the first"
+
+
+@pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
+@pytest.mark.parametrize("m,n,k", [(8, 1000, 3584), (3, 520, 4104), (16, 264, 8200), (1, 18944, 512)])
+def test_gemv_back_to_back_under_pdl_is_bit_stable(layout, m, n, k):
+    """decode_gemv launches with programmatic stream serialization: call i + 1 prefetches W while call i drains.  X and Y are
+    touched only after the previous grid completed; alternating two weight matrices and 32 outputs checks exactly that."""
+    x = normal_bf16(97, (m, k))
+    ws = [normal_bf16(98 + j, (k, n), 0.05) for j in range(2)]
+    wps = [np.ascontiguousarray(w.T if layout == tri.TRI_W_NK else w) for w in ws]
+    ldw = wps[0].shape[1]
+    if ldw % 8:                                           # TRI_W_KN with ragged n: pad the rows
+        pad = (-ldw) % 8
+        wps = [np.concatenate([p, np.full((p.shape[0], pad), NAN16, np.uint16)], axis=1) for p in wps]
+        ldw += pad
+    dx, dws = dev(x), [dev(p) for p in wps]
+    reps = 32
+    outs = [torch.full((m, n), NAN16, dtype=torch.int16, device="cuda") for _ in range(reps)]
+    for i, y in enumerate(outs):
+        tri.decode_gemv(m, n, k, dx, k, dws[i & 1], ldw, layout, y, n)
+    torch.cuda.synchronize()
+    for j in range(2):
+        ref = outs[j].cpu().numpy().view(np.uint16)
+        within_bound(ref, x, np.ascontiguousarray(wps[j][:, :(k if layout == tri.TRI_W_NK else n)]), layout)
+        for i in range(j + 2, reps, 2):
+            assert torch.equal(outs[i], outs[j]), f"call {i} differs from call {j}"
+
+
+def test_gemv_then_gemm_then_gemv_chain():
+    """The bench step's order: PDL-launched GEMVs around a (split) GEMM and its reduction kernel on one stream."""
+    m, n, k = 8, 1096, 2048
+    x, w = normal_bf16(101, (m, k)), normal_bf16(102, (k, n), 0.05)
+    a = normal_bf16(103, (300, k))
+    wp = np.ascontiguousarray(w.T)
+    dx, dw, da = dev(x), dev(wp), dev(a)
+    ys = [torch.full((m, n), NAN16, dtype=torch.int16, device="cuda") for _ in range(12)]
+    cs = [torch.full((300, n), NAN16, dtype=torch.int16, device="cuda") for _ in range(6)]
+    for i in range(6):
+        tri.decode_gemv(m, n, k, dx, k, dw, k, tri.TRI_W_NK, ys[2 * i], n)
+        tri.prefill_gemm(300, n, k, da, k, dw, k, tri.TRI_W_NK, cs[i], n)       # 2 x 5 tiles < 74 pairs: split, reduction kernel
+        tri.decode_gemv(m, n, k, dx, k, dw, k, tri.TRI_W_NK, ys[2 * i + 1], n)
+    torch.cuda.synchronize()
+    within_bound(ys[0].cpu().numpy().view(np.uint16), x, wp, tri.TRI_W_NK)
+    within_bound(cs[0].cpu().numpy().view(np.uint16), a, wp, tri.TRI_W_NK)
+    assert all(torch.equal(y, ys[0]) for y in ys) and all(torch.equal(c, cs[0]) for c in cs)

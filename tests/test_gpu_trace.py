@@ -59,7 +59,7 @@ def test_phase_trace_driver_short():
     names = [s["phase_name"] for s in summ]
     assert names == (["prefill", "decode", "idle"] * 2)[:len(names)] and len(names) >= 5   # phases overrun by a launch or two:
                                                                                          # the last idle may be cut at total_s
-    assert 80 <= len(samples) <= 230
+    assert 0.9 * 2.0 / 0.010 <= len(samples) <= 230           # the 10 ms period of config 5 is held (energy is refreshed every 100 ms)
     for i, s in enumerate(summ):
         assert s["t_end_s"] > s["t_begin_s"]
         if s["phase_name"] == "idle":
@@ -69,7 +69,7 @@ def test_phase_trace_driver_short():
         else:
             assert s["launches"] > 10 and s["gpu_ms"] > 300
             assert s["energy_j"] > 0 and s["j_per_flop"] > 0 and s["j_per_token"] > 0
-            assert s["n_samples"] >= 12 and s["sm_mhz_mean"] > 0      # 40 nominal; NVML queries contend with the launch path
+            assert s["n_samples"] >= 0.8 * 40 and s["sm_mhz_mean"] > 0      # 0.4 s / 10 ms = 40 nominal
             per = 2.0 * (pm * pn * pk if s["phase_name"] == "prefill" else dm * dn * dk)
             assert abs(s["flop"] - per * s["launches"]) < 1e-3 * s["flop"]
     # the sampler tagged samples with the phase the driver was in
@@ -78,3 +78,52 @@ def test_phase_trace_driver_short():
     # and the GEMM output of the last prefill call is the real product (spot check)
     ref = pa[:64].float() @ pw.float().T
     assert (pc[:64].float() - ref).abs().max().item() < 0.05
+
+
+def test_prefill_clock_decay_is_reported():
+    """Fig. 4a: inside one prefill window the clock decays.  On B200 the config-4 GEMM starts at the
+    boost ceiling and is pulled down by the 1000 W cap within the first few hundred ms (profiles/r1_trace60.md: 1684 ->
+    1307 MHz); the per-phase summary must show it as first-10 % > last-10 %, and the decode phase must run at a higher
+    clock than the end of the prefill phase (Observation 2)."""
+    pm, pn, pk = 4096, 18944, 3584
+    dm, dn, dk = 8, 18944, 3584
+    pa = normal_bf16_torch(4, (pm, pk), 1.0, "cuda", stream=0)
+    pw = normal_bf16_torch(4, (pn, pk), 0.02, "cuda", stream=1)
+    pc = torch.empty((pm, pn), dtype=torch.bfloat16, device="cuda")
+    dx = normal_bf16_torch(4, (dm, dk), 1.0, "cuda", stream=2)
+    dws = [normal_bf16_torch(4, (dn, dk), 0.02, "cuda", stream=3 + r) for r in range(8)]
+    dy = torch.empty((dm, dn), dtype=torch.bfloat16, device="cuda")
+    torch.cuda.synchronize()
+    time.sleep(1.0)                                            # start from an idle, cool-ish part as config 5's idle gap does
+    samples, summ = tri.phase_trace(pm, pn, pk, pa, pw, pc, dm, dn, dk, dx, dws, dy, tri.TRI_W_NK, total_s=3.0,
+                                    prefill_s=1.5, decode_s=1.0, idle_s=0.5, period_ms=10)
+    assert len(samples) >= 0.9 * 3.0 / 0.010
+    pre, dec = summ[0], summ[1]
+    assert pre["phase_name"] == "prefill" and dec["phase_name"] == "decode"
+    assert pre["n_samples"] >= 0.8 * 150 and dec["n_samples"] >= 0.8 * 100
+    assert pre["sm_mhz_first10"] > pre["sm_mhz_last10"], (pre["sm_mhz_first10"], pre["sm_mhz_last10"])
+    assert dec["sm_mhz_mean"] > pre["sm_mhz_last10"], (dec["sm_mhz_mean"], pre["sm_mhz_last10"])
+    assert pre["mean_power_w"] > 500 and dec["mean_power_w"] > 500 and pre["j_per_flop"] < 0.1 * dec["j_per_flop"]
+
+
+def test_characterise_thermal_short(tmp_path):
+    """Row f2's built half: `characterise thermal` on two points for 3 s each; every 1 s bin carries
+    throughput, clock, temperature and power, and the rates are the kernels' own."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = tmp_path / "thermal.json"
+    r = subprocess.run([sys.executable, "-m", "paper_2606_29629_b200.characterise", "thermal", "--seconds", "3", "--cooldown", "0",
+                        "--points", "k16,gemv", "--out", str(out)], cwd=root, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    doc = json.load(open(out))
+    assert [p["point"] for p in doc["points"]] == ["k16", "gemv"]
+    for p in doc["points"]:
+        assert p["series_columns"] == ["t_s", "tflops", "gbs", "sm_mhz", "temp_c", "power_w"]
+        assert len(p["series"]) >= 2 and p["calls"] > 100
+        for sec, tflops, gbs, mhz, temp, watts in p["series"]:
+            assert tflops > 0 and 4500 < gbs < 7500 and 500 <= mhz <= 2100 and 20 <= temp <= 100 and 100 < watts < 1100
+        assert p["j_per_flop"] and p["j_per_flop"] > 0 and p["tflops_first"] and p["sm_mhz_last"]
+    assert doc["points"][0]["ai"] == 4.0 and abs(doc["points"][1]["ai"] - 7.98) < 0.01
