@@ -10,6 +10,11 @@
 //     slots; full / empty mbarriers.  X rides in the ring, so there is no prologue, no limit on K, and nothing but
 //     the ring in shared memory.
 //
+//   * few columns (N / 64 < 148 CTAs, e.g. the down-projection 18944 -> 3584: 56 column blocks): the launch is a grid of
+//     CTA CLUSTERS along K — cluster rank r streams stages [r S'/S, (r+1) S'/S) of the same 64 columns, writes its fp32
+//     partial sums into its own (by then dead) ring, and after a cluster barrier rank 0 adds the S partials in rank order
+//     through distributed shared memory (ld.shared::cluster) and stores.  No workspace, no second kernel, fixed order.
+//
 // Two arithmetic paths behind it:
 //
 // (1) m <= 4: CUDA cores, the sm_100 mixed-precision FMA  fma.rn.f32.bf16  (SASS FHFMA.BF16): d = a * b + c with a, b
@@ -132,9 +137,10 @@ __device__ __forceinline__ GemvBars gemv_setup(uint8_t *smem_raw, int nslots, ui
 // Producer (one lane): streams the CTA's weight panel and the matching X slices through the ring.  W (model state,
 // never an output of the preceding kernel) is fetched at once; X is fetched only after pdl_wait(), i.e. after the
 // preceding grid has completed (aliasing rule in include/triroof.h).
+// Stages [s0, s0 + nstages) of the K range belong to this CTA (the whole range unless the launch is a K-split cluster).
 template <int SLOT_BYTES, bool KN>
 __device__ __forceinline__ void gemv_producer(const GemvBars &b, const CUtensorMap *wmap, const CUtensorMap *xmap, int n0,
-                                              int nstages, int nslots)
+                                              int s0, int nstages, int nslots)
 {
     ptx::prefetch_tmap(wmap);
     ptx::prefetch_tmap(xmap);
@@ -144,23 +150,63 @@ __device__ __forceinline__ void gemv_producer(const GemvBars &b, const CUtensorM
     for (int s = 0; s < npre; ++s) {
         const uint32_t fb = b.full0 + 8 * s;
         ptx::mbar_arrive_expect_tx(fb, SLOT_BYTES);
-        if (KN) ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, n0, s * GV_STAGE_K, fb, pol_w);
-        else ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, s * GV_STAGE_K, n0, fb, pol_w);
+        if (KN) ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, n0, (s0 + s) * GV_STAGE_K, fb, pol_w);
+        else ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES, wmap, (s0 + s) * GV_STAGE_K, n0, fb, pol_w);
     }
     ptx::pdl_wait();
     for (int s = 0; s < npre; ++s)
-        ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES + GV_W_BYTES, xmap, s * GV_STAGE_K, 0, b.full0 + 8 * s, pol_x);
+        ptx::tma_load_2d_hint(b.ring + s * SLOT_BYTES + GV_W_BYTES, xmap, (s0 + s) * GV_STAGE_K, 0, b.full0 + 8 * s, pol_x);
     int slot = 0;
     uint32_t par = 0;                                          // parity of the slot's first release
     for (int s = npre; s < nstages; ++s) {
         ptx::mbar_wait(b.empty0 + 8 * slot, par);
         const uint32_t fb = b.full0 + 8 * slot, dst = b.ring + slot * SLOT_BYTES;
         ptx::mbar_arrive_expect_tx(fb, SLOT_BYTES);
-        if (KN) ptx::tma_load_2d_hint(dst, wmap, n0, s * GV_STAGE_K, fb, pol_w);
-        else ptx::tma_load_2d_hint(dst, wmap, s * GV_STAGE_K, n0, fb, pol_w);
-        ptx::tma_load_2d_hint(dst + GV_W_BYTES, xmap, s * GV_STAGE_K, 0, fb, pol_x);
+        if (KN) ptx::tma_load_2d_hint(dst, wmap, n0, (s0 + s) * GV_STAGE_K, fb, pol_w);
+        else ptx::tma_load_2d_hint(dst, wmap, (s0 + s) * GV_STAGE_K, n0, fb, pol_w);
+        ptx::tma_load_2d_hint(dst + GV_W_BYTES, xmap, (s0 + s) * GV_STAGE_K, 0, fb, pol_x);
         if (++slot == nslots) { slot = 0; par ^= 1; }
     }
+}
+
+// K-split clusters: this CTA's share of the stages and of the column blocks.
+struct GemvSplit {
+    uint32_t rank, nranks;     // position in the cluster along K (0, 1 when the launch has no clusters)
+    int n0, s0, nstages;
+};
+__device__ __forceinline__ GemvSplit gemv_split(int k)
+{
+    GemvSplit g;
+    g.rank = ptx::cluster_ctarank();
+    g.nranks = ptx::cluster_nctarank();
+    g.n0 = (int)(blockIdx.x / g.nranks) * GV_COLS;
+    const int total = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+    g.s0 = (int)((int64_t)g.rank * total / g.nranks);
+    g.nstages = (int)((int64_t)(g.rank + 1) * total / g.nranks) - g.s0;
+    return g;
+}
+constexpr uint32_t GV_PART_OFFSET = 20480;      // partial sums of a K-split rank, inside its ring (beyond the FHFMA path's 17 KiB of sets)
+// Rank 0 adds the partials of ranks 1 .. nranks - 1 (written at `part` + 16 * tid * VEC in each rank's own ring) to `v`, in
+// rank order.  Every thread of every CTA of the cluster calls this (two cluster barriers).
+template <int VEC>
+__device__ __forceinline__ void gemv_cluster_reduce(const GemvSplit &g, uint32_t part, bool compute_thread, float4 (&v)[VEC])
+{
+    if (compute_thread && g.rank != 0) {
+#pragma unroll
+        for (int i = 0; i < VEC; ++i)
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(part + 16 * (threadIdx.x * VEC + i)), "f"(v[i].x), "f"(v[i].y),
+                         "f"(v[i].z), "f"(v[i].w) : "memory");
+    }
+    ptx::cluster_sync();                                              // partials are written (release / acquire at cluster scope)
+    if (compute_thread && g.rank == 0) {
+        for (uint32_t r = 1; r < g.nranks; ++r)
+#pragma unroll
+            for (int i = 0; i < VEC; ++i) {
+                const float4 o = ptx::ld_shared_cluster_f4(part + 16 * (threadIdx.x * VEC + i), r);
+                v[i].x += o.x; v[i].y += o.y; v[i].z += o.z; v[i].w += o.w;
+            }
+    }
+    ptx::cluster_sync();                                              // nobody leaves while rank 0 reads its shared memory
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -179,11 +225,16 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
     const uint32_t ring = b.ring, full0 = b.full0, empty0 = b.empty0;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * GV_COLS;
-    const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+    const GemvSplit g = gemv_split(k);
+    const int n0 = g.n0, nstages = g.nstages;
 
     if (warp == GV_CWARPS) {
-        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, nstages, nslots);
+        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, g.s0, nstages, nslots);
+        if (g.nranks > 1) {
+            __syncwarp();
+            float4 none[1];
+            gemv_cluster_reduce<1>(g, 0, false, none);
+        }
         return;
     }
 
@@ -284,15 +335,23 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
             for (int mm = 0; mm < MR; ++mm) mine[mm * GV_COLS + 16 * j] = acc[j][mm];
     }
     asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");
-    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
     const int mm = threadIdx.x >> 4, col = (threadIdx.x & 15) * 4;    // 16 threads x 4 outputs per row of 64 columns
-    if (mm < m && mm < MR && n0 + col < n) {
-        float4 sum = make_float4(0.f, 0.f, 0.f, 0.f);
+    const bool valid = mm < m && mm < MR && n0 + col < n;
+    float4 tot[1] = {make_float4(0.f, 0.f, 0.f, 0.f)};
+    if (valid) {
 #pragma unroll
         for (int t = 0; t < NSETS; ++t) {
             const float4 v = *reinterpret_cast<const float4 *>(red + (size_t)t * GV_RED_STRIDE + mm * GV_COLS + col);
-            sum.x += v.x; sum.y += v.y; sum.z += v.z; sum.w += v.w;
+            tot[0].x += v.x; tot[0].y += v.y; tot[0].z += v.z; tot[0].w += v.w;
         }
+    }
+    if (g.nranks > 1) {                                               // K-split cluster: rank 0 collects the other ranks' sums
+        gemv_cluster_reduce<1>(g, ring + GV_PART_OFFSET, true, tot);
+        if (g.rank != 0) return;
+    }
+    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
+    if (valid) {
+        const float4 sum = tot[0];
         uint16_t *dst = y + (int64_t)mm * ldy + n0 + col;
         const uint32_t lo = ptx::pack_bf16x2(sum.x, sum.y), hi = ptx::pack_bf16x2(sum.z, sum.w);
         if (n0 + col + 4 <= n && (reinterpret_cast<uintptr_t>(dst) & 7) == 0) {
@@ -321,11 +380,16 @@ gemv_mma_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
     const GemvBars b = gemv_setup<SLOT>(smem_raw, nslots, &smem);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int n0 = blockIdx.x * GV_COLS;
-    const int nstages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+    const GemvSplit g = gemv_split(k);
+    const int n0 = g.n0, nstages = g.nstages;
 
     if (warp == GV_CWARPS) {
-        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, nstages, nslots);
+        if (lane == 0) gemv_producer<SLOT, KN>(b, &wmap, &xmap, n0, g.s0, nstages, nslots);
+        if (g.nranks > 1) {
+            __syncwarp();
+            float4 none[NT];
+            gemv_cluster_reduce<NT>(g, 0, false, none);
+        }
         return;
     }
 
@@ -374,26 +438,36 @@ gemv_mma_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
             for (int t = 0; t < NT; ++t) mma_16816(acc[ks & 1][t], af[ks], bf[t][ks >> 1][2 * (ks & 1)], bf[t][ks >> 1][2 * (ks & 1) + 1]);
     }
 
-    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
-    const int g = lane >> 2, t4 = lane & 3;
+    float4 tot[NT];
 #pragma unroll
     for (int t = 0; t < NT; ++t)
+        tot[t] = make_float4(acc[0][t][0] + acc[1][t][0], acc[0][t][1] + acc[1][t][1], acc[0][t][2] + acc[1][t][2], acc[0][t][3] + acc[1][t][3]);
+    if (g.nranks > 1) {                                               // K-split cluster: rank 0 collects the other ranks' sums
+        asm volatile("bar.sync 1, %0;" ::"n"(GV_CTHREADS) : "memory");   // every warp of this CTA is done with the ring
+        gemv_cluster_reduce<NT>(g, b.ring + GV_PART_OFFSET, true, tot);
+        if (g.rank != 0) return;
+    }
+    ptx::pdl_wait();                                                  // Y may be read by the preceding kernel
+    const int gq = lane >> 2, t4 = lane & 3;
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        const float d[4] = {tot[t].x, tot[t].y, tot[t].z, tot[t].w};
 #pragma unroll
         for (int h = 0; h < 2; ++h) {                                 // D rows g, g + 8 = output columns
-            const int col = n0 + 16 * warp + g + 8 * h;
+            const int col = n0 + 16 * warp + gq + 8 * h;
 #pragma unroll
             for (int e = 0; e < 2; ++e) {                             // D columns 2t, 2t + 1 = batch rows
                 const int row = 8 * t + 2 * t4 + e;
-                if (col < n && row < m)
-                    y[(int64_t)row * ldy + col] =
-                        __bfloat16_as_ushort(__float2bfloat16_rn(acc[0][t][2 * h + e] + acc[1][t][2 * h + e]));
+                if (col < n && row < m) y[(int64_t)row * ldy + col] = __bfloat16_as_ushort(__float2bfloat16_rn(d[2 * h + e]));
             }
         }
+    }
 }
 
+// ksplit > 1: a grid of CTA clusters of that size along K (see the file header).
 template <typename Kernel>
 static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y,
-                               int64_t ldy, int m, int n, int k, int nslots, int blocks, cudaStream_t s)
+                               int64_t ldy, int m, int n, int k, int nslots, int blocks, int ksplit, cudaStream_t s)
 {
     if (*attr_gen != device_generation()) {       // per-device function attribute: redo after tri_init() moved to another device
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS, 16));
@@ -401,29 +475,33 @@ static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CU
         *attr_gen = device_generation();
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(blocks);
+    cfg.gridDim = dim3(blocks * ksplit);
     cfg.blockDim = dim3(GV_THREADS);
     cfg.dynamicSmemBytes = gemv_smem_bytes(nslots, xrows);
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = ksplit;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = ksplit > 1 ? 2 : 1;
     return cudaLaunchKernelEx(&cfg, kernel, wmap, xmap, y, ldy, m, n, k, nslots);
 }
 
 // Row-count dispatch.  One static generation counter per instantiation (function attributes are per device).
 template <bool KN>
 static cudaError_t launch_gemv_rows(int m, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
-                                    int nslots, int blocks, cudaStream_t s)
+                                    int nslots, int blocks, int ksplit, cudaStream_t s)
 {
     static int gen[5] = {-1, -1, -1, -1, -1};
-    if (m <= 1) return launch_gemv(gemv_kernel<1, KN>, &gen[0], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
-    if (m <= 2) return launch_gemv(gemv_kernel<2, KN>, &gen[1], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
-    if (m <= 4) return launch_gemv(gemv_kernel<4, KN>, &gen[2], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
-    if (m <= 8) return launch_gemv(gemv_mma_kernel<1, KN>, &gen[3], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
-    return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, s);
+    if (m <= 1) return launch_gemv(gemv_kernel<1, KN>, &gen[0], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    if (m <= 2) return launch_gemv(gemv_kernel<2, KN>, &gen[1], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    if (m <= 4) return launch_gemv(gemv_kernel<4, KN>, &gen[2], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    if (m <= 8) return launch_gemv(gemv_mma_kernel<1, KN>, &gen[3], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
 }
 
 static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
@@ -469,11 +547,21 @@ static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const 
     // slots also fill the SM with two CTAs, so that no CTA of the NEXT call (programmatic dependent launch) moves in early
     // and spins on its barriers in the issue slots of the running ones.  The FHFMA path's partial-sum sets reuse the ring.
     const int nslots = GV_MAX_SLOTS;
-    static_assert((size_t)GV_MAX_SLOTS * gemv_slot_bytes(8) >= (size_t)16 * GV_RED_STRIDE * 4, "the partial sums must fit the ring");
+    static_assert((size_t)GV_MAX_SLOTS * gemv_slot_bytes(8) >= GV_PART_OFFSET + 4096 && GV_PART_OFFSET >= (size_t)16 * GV_RED_STRIDE * 4,
+                  "the partial sums must fit the ring");
     static_assert(2 * gemv_smem_bytes(GV_MAX_SLOTS, 16) <= 227 * 1024, "two CTAs per SM");
 
-    cudaError_t e = kn ? launch_gemv_rows<true>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, s)
-                       : launch_gemv_rows<false>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, s);
+    // Fewer column blocks than two per SM: clusters of 2 or 4 along K, as long as a rank keeps at least 24 stages (a CTA's
+    // fixed cost is worth ~10 stages).  Measured on 8 x 3584 x 18944 (56 column blocks): 1 / 2 / 3 / 4 / 5 / 6 / 8 ranks ->
+    // 39.6 / 25.8 / 22.4 / 21.6 / 27.4 / 26.6 / 24.1 us (sizes that do not pack the GPCs evenly run in two waves); on
+    // 8 x 4608 x 3584 (56 stages in all): 9.0 / 8.7 / 8.2 / 11.0 us for 1 / 2 / 3 / 4.
+    const int total_stages = (k + GV_STAGE_K - 1) / GV_STAGE_K;
+    const int room = (2 * di->sm_count) / blocks;
+    int ksplit = room >= 4 ? 4 : room >= 2 ? 2 : 1;
+    while (ksplit > 1 && total_stages / ksplit < 24) ksplit /= 2;
+
+    cudaError_t e = kn ? launch_gemv_rows<true>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, ksplit, s)
+                       : launch_gemv_rows<false>(m, wmap, xmap, y, ldy, n, k, nslots, blocks, ksplit, s);
     if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "decode_gemv launch: %s", cudaGetErrorString(e));
     return TRI_OK;
 }

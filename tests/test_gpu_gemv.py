@@ -66,7 +66,7 @@ def test_config3_full_output(layout):
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
-@pytest.mark.parametrize("m", [1, 4, 5, 16])
+@pytest.mark.parametrize("m", [1, 2, 4, 5, 16])
 def test_config3_shape_other_batch_sizes(layout, m):
     """The config-3 weight matrix at the other decode batch sizes: m = 1, 4 run the FHFMA kernels,
     m = 5 the warp-MMA kernel with zero-filled rows, m = 16 its two-tile form; full output, stated bound."""
@@ -79,10 +79,11 @@ def test_config3_shape_other_batch_sizes(layout, m):
 
 
 @pytest.mark.parametrize("layout", [tri.TRI_W_NK, tri.TRI_W_KN])
-@pytest.mark.parametrize("m", [5, 8, 16])
+@pytest.mark.parametrize("m", [1, 2, 4, 5, 8, 16])
 def test_down_projection_shape_full_output(layout, m):
-    """The Thinker MLP down-projection at decode batch sizes (18944 -> 3584): K = 18944 = 296 stages
-    through the 10-slot ring, every row count of the warp-MMA path; full output, stated bound."""
+    """The Thinker MLP down-projection at decode batch sizes (18944 -> 3584): 56 column blocks, so the launch
+    is a grid of 5-CTA clusters along K (59-60 stages per rank through the 10-slot ring, partial sums through distributed
+    shared memory); every kernel of both paths; full output, stated bound."""
     k, n = 18944, 3584
     x = normal_bf16(2, (m, k), 1.0, stream=8)
     w = normal_bf16(2, (k, n), 0.02, stream=9)
