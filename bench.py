@@ -151,10 +151,10 @@ def run_reference(args):
 
 
 def workload_config(n_gpus):
-    return {"workload": "configs[1] A.I. sweep (FMA chain N=2^28 fp32, k=2^0..2^12) + configs[2] decode GEMV 8x3584x18944 "
-                        "x 8 rotating W copies + configs[3] prefill GEMM 4096x3584x18944; W layout NK",
+    return {"workload": "configs[1] FMA-chain A.I. sweep N=2^28 k=2^0..2^12 + configs[2] GEMV 8x3584x18944 x 8 W copies "
+                        "+ configs[3] GEMM 4096x3584x18944; W layout NK",
             "parallelism": f"replicas x{n_gpus} (no collective)",
-            "l2": "inputs larger than L2 (2 GiB stream; 8 x 136 MB GEMV weights, copy 0 = the configured W; 320 MB GEMM operands)"}
+            "l2": "inputs larger than L2 (2 GiB stream; 8 x 136 MB rotating W; 320 MB GEMM operands)"}
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -375,7 +375,7 @@ def gemm_shape_series(torch, tri, peaks):
     return out
 
 
-UNIT = "TFLOP/s (algorithmic, whole step: fp32-FMA + bf16-tensor FLOP)"
+UNIT = "TFLOP/s (algorithmic, whole step: fp32 FMA + bf16 tensor)"
 DETAIL_FILE = os.path.join("gpurun_out", "bench_points.json")
 COMPACT_KEYS = ["impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
                 "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "min_frac"]
@@ -394,23 +394,26 @@ def sig(x, digits=4):
 def compact_line(full):
     """The ONE line of stdout: the bench contract's keys, plus the metric BASELINE.json names in compact form —
     `fracs` = fraction of roofline per A.I. point (burst, per-launch CUDA-event medians of the timed steps) and
-    `sustained` = per point [fraction of the roofline at the recorded clock, SM MHz, W, pJ/FLOP] from the looped pass
+    `sustained` = per point, in the order of `fracs`, [fraction of the roofline at the recorded clock, SM MHz, W, pJ/FLOP] from the looped pass
     (the ridge and paper-A.I. extra series are in the detail file only).
-    Everything bulky (`points`, `extra_points`, `model_fit`) stays in the detail file.  Kept under 3 KB: the round-1
-    line was 20 KB and the driver could not parse it."""
+    Everything bulky (`points`, `extra_points`, `model_fit`) stays in the detail file.  Kept near 2 KB: the round-1
+    line was 20 KB and the driver, which reads the last 3000 bytes of stdout, could not parse it."""
     out = {k: full[k] for k in COMPACT_KEYS if k in full}
     pts = full.get("points") or []
     out["fracs"] = {point_key(p): round(p["frac"], 3) for p in pts}
-    sus = {}
+    def short(x, digits):                                             # 640.0 -> 640 on the line
+        x = sig(x, digits)
+        return int(x) if x is not None and x >= 100 else x
+    sus = []
     for p in pts:
         c = p.get("sustained")
         if c and p.get("frac_sustained_at_clock") is not None:
             pj = c.get("j_per_flop")
-            sus[point_key(p)] = [round(p["frac_sustained_at_clock"], 3), int(c.get("sm_mhz") or 0), int(c.get("power_w_mean") or 0),
-                                 sig(pj * 1e12 if pj else None, 3)]
-    if sus:
+            sus.append([round(p["frac_sustained_at_clock"], 2), int(c.get("sm_mhz") or 0), int(c.get("power_w_mean") or 0),
+                        short(pj * 1e12 if pj else None, 2)])
+    if len(sus) == len(pts) and sus:
         out["sustained"] = sus
-        out["sustained_cols"] = "frac at recorded clock, SM MHz, W, pJ/FLOP"
+        out["sustained_cols"] = "in the order of fracs: frac at clock, SM MHz, W, pJ/FLOP"
     gm = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "prefill_gemm" and q.get("label")]
     if gm:
         out["gemm_shapes"] = {q["label"]: round(q["frac"], 3) for q in gm}
@@ -418,9 +421,9 @@ def compact_line(full):
         out["j_per_flop"] = sig(full["energy"].get("j_per_flop"), 3)
     out["detail"] = DETAIL_FILE
 
-    def rounded(x):                                                   # 6 significant digits are plenty on the line; the file has them all
+    def rounded(x):                                                   # 5 significant digits are plenty on the line; the file has them all
         if isinstance(x, float):
-            return sig(x, 6)
+            return sig(x, 5)
         if isinstance(x, dict):
             return {k: rounded(v) for k, v in x.items()}
         if isinstance(x, list):
@@ -605,8 +608,8 @@ def run_ours(args):
     roofline = {"kernel": "fma_chain_kernel (k=4096 launch)", "bound": "alu", "achieved": dom["tflops"], "peak": alu_peak,
                 "unit": "TFLOP/s", "frac": dom["tflops"] / alu_peak, "traffic": traffic,
                 "share_of_step": dom["ms"] * args.steps / total_ms,
-                "peak_source": f"derived {sms} SMs x {FP32_LANES_PER_SM} lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz; fracs: {peaks['source']} "
-                               f"{peaks['hbm_gbs']} GB/s, {peaks['bf16_tflops']} TFLOP/s"}
+                "peak_source": f"derived {sms} SMs x {FP32_LANES_PER_SM} x 2 x {peaks['sm_max_mhz']:.0f} MHz; fracs vs {peaks['source']} "
+                               f"{peaks['hbm_gbs']:.0f} GB/s, {peaks['bf16_tflops']:.0f} TF/s"}
 
     # ---- end to end: host buffers in, host buffers out, copies inside the timed region ----
     e2e = run_e2e(torch, tri, step, args, barrier, dist)
@@ -707,7 +710,7 @@ def run_e2e(torch, tri, step, args, barrier, dist):
     world = dist.get_world_size() if dist is not None else 1
     return {"value": whole_job_value(STEP_FLOP, n, world, ms), "unit": UNIT,
             "ms_per_step": ms / n, "steps": n, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-            "overlap": "H2D(i+1) | kernels(i) | D2H(i-1)", "readback_checked": ok}
+            "overlap": "H2D(i+1)|kernels(i)|D2H(i-1)", "readback_checked": ok}
 
 
 def main():
