@@ -118,7 +118,12 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
  * m, n >= 1; k >= 8, k % 8 == 0.  a: device bf16 A[i * lda + kk], lda >= k, lda % 8 == 0.
  * w: as in decode_gemv.  c: device bf16 C[i * ldc + j], ldc >= n, ldc % 8 == 0.
  * a, w, c 16-byte aligned.  Ragged m, n, k tiles are handled inside (TMA zero fill, clipped stores).
- * Outputs must not alias inputs.  Asynchronous: one kernel on `stream`.
+ * Outputs must not alias inputs.  Asynchronous: one kernel on `stream` (two when the shape is split along k: the
+ * second adds the fp32 partial tiles in a fixed order).
+ * For m <= 128 the kernel is launched with programmatic stream serialization, like decode_gemv: it prefetches W
+ * (model state) while the kernel before it on `stream` drains, and reads A / writes C only after that kernel has
+ * completed.  W must therefore not be an output of the immediately preceding prefill_gemm / decode_gemv call on
+ * the same stream (any other producer of W is ordered as usual).
  */
 int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
                  int w_layout, uint16_t *c, int64_t ldc, void *stream);

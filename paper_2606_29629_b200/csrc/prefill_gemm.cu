@@ -12,6 +12,10 @@
 // MMA issuer (tcgen05.mma.cta_group::1.kind::f16, M 128, N 128, K 16), warp 2 TMEM owner (two 128-column accumulators),
 // warps 4-7 epilogue (tcgen05.ld -> cvt.rn.bf16x2 -> 16-byte global stores; the output is small here).
 // Ragged M / N / K: TMA zero-fills out-of-bounds reads; stores clip.
+// Programmatic dependent launch, as in the GEMV: the kernel lets the next kernel of the stream start at once and orders
+// itself with griddepcontrol.wait — the producer fetches a ring-full of W (model state) before the wait and A after it,
+// the epilogue waits before its first store.  Back to back on m x 18944 x 3584: m = 16 / 64 / 128 26.9 / 26.7 / 27.5 us
+// -> 23.7 / 23.9 / 25.3 us (cuBLAS 25.5 / 28.2 / 28.9).
 //
 // W layouts: TRI_W_NK is the K-major B operand (canonical).  TRI_W_KN is the MN-major B operand: the W tile is loaded
 // as 64(n) x 64(k) boxes and described to the MMA with the MN-major descriptor.
@@ -49,7 +53,9 @@ gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int ntiles = p.tiles_m * p.tiles_n, me = blockIdx.x, nw = gridDim.x;
 
-    if (p.parts > 1) ptx::pdl_launch_dependents();        // splitk_reduce_kernel may take its place; it waits for this grid
+    // Programmatic dependent launch: the next kernel of the stream (splitk_reduce_kernel when this call is split, else the
+    // next call's kernel) may start its CTAs as soon as resources free up; it orders itself with griddepcontrol.wait.
+    ptx::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < GM_STAGES; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);
@@ -72,29 +78,45 @@ gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
 
     if (warp == 0) {
         // ===== TMA producer =====
+        // W (model state, never an output of the kernel before this one) is fetched at once for the first ring-full of
+        // k-blocks; A is fetched only after griddepcontrol.wait, i.e. once the preceding grid has completed (header:
+        // aliasing rule).  Then the steady loop.
         if (ptx::elect_one()) {
             ptx::prefetch_tmap(&amap);
             ptx::prefetch_tmap(&wmap);
             const uint64_t pol_w = ptx::policy_evict_first();        // every W element is read exactly once
             const uint64_t pol_a = ptx::policy_evict_last();         // A is re-read by every CTA
-            uint32_t it = 0;
+            auto load_w = [&](uint32_t sb, uint32_t fb, int tn, int kb) {
+                if (!p.b_mn_major) {
+                    ptx::tma_load_2d_hint(sb, &wmap, kb * GM_BK, tn * GM_BN, fb, pol_w);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < GM_BN / 64; ++q)   // 64(n) x 64(k) boxes, 8 KiB each
+                        ptx::tma_load_2d_hint(sb + q * 8192, &wmap, tn * GM_BN + q * 64, kb * GM_BK, fb, pol_w);
+                }
+            };
             GemmWork wk;
+            uint32_t it = 0;
+            for (int i = 0; it < (uint32_t)GM_STAGES && next_work(p, ntiles, me, nw, i, wk); ++i)
+                for (int kb = wk.kb0; kb < wk.kb1 && it < (uint32_t)GM_STAGES; ++kb, ++it) {
+                    const uint32_t fb = full0 + 8 * it;
+                    ptx::mbar_arrive_expect_tx(fb, GM_STAGE_BYTES);
+                    load_w(ring + it * GM_STAGE_BYTES + GM_A_BYTES, fb, wk.tile / p.tiles_m, kb);
+                }
+            ptx::pdl_wait();
+            it = 0;
             for (int i = 0; next_work(p, ntiles, me, nw, i, wk); ++i) {
                 const int tm = wk.tile % p.tiles_m, tn = wk.tile / p.tiles_m;
                 for (int kb = wk.kb0; kb < wk.kb1; ++kb, ++it) {
                     const uint32_t s = it % GM_STAGES, ph = (it / GM_STAGES) & 1;
-                    ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);
                     const uint32_t fb = full0 + 8 * s;
-                    ptx::mbar_arrive_expect_tx(fb, GM_STAGE_BYTES);
                     const uint32_t sa = ring + s * GM_STAGE_BYTES, sb = sa + GM_A_BYTES;
-                    ptx::tma_load_2d_hint(sa, &amap, kb * GM_BK, tm * GM_BM, fb, pol_a);
-                    if (!p.b_mn_major) {
-                        ptx::tma_load_2d_hint(sb, &wmap, kb * GM_BK, tn * GM_BN, fb, pol_w);
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < GM_BN / 64; ++q)   // 64(n) x 64(k) boxes, 8 KiB each
-                            ptx::tma_load_2d_hint(sb + q * 8192, &wmap, tn * GM_BN + q * 64, kb * GM_BK, fb, pol_w);
+                    if (it >= (uint32_t)GM_STAGES) {
+                        ptx::mbar_wait(empty0 + 8 * s, ph ^ 1);
+                        ptx::mbar_arrive_expect_tx(fb, GM_STAGE_BYTES);
+                        load_w(sb, fb, tn, kb);
                     }
+                    ptx::tma_load_2d_hint(sa, &amap, kb * GM_BK, tm * GM_BM, fb, pol_a);
                 }
             }
         }
@@ -130,6 +152,7 @@ gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         const int ew = warp & 3;                                      // TMEM lanes 32*ew .. 32*ew+31
         uint32_t tcount = 0;
         GemmWork wk;
+        ptx::pdl_wait();                                              // C / the workspace may still be in use by the preceding grid
         for (int i = 0; next_work(p, ntiles, me, nw, i, wk); ++i, ++tcount) {
             const int tm = wk.tile % p.tiles_m, tn = wk.tile / p.tiles_m;
             const uint32_t acc = tcount & 1, aph = (tcount >> 1) & 1;
@@ -201,6 +224,7 @@ gemm_1sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
 __global__ void __launch_bounds__(256)
 splitk_reduce_kernel(const GemmParams p, int tile_rows, int tile_cols, int pair_order)
 {
+    ptx::pdl_launch_dependents();                          // the next call may set itself up; it waits for this grid before touching C / ws
     ptx::pdl_wait();                                       // the GEMM kernel's partial tiles are complete and visible
     const int ntiles = p.tiles_m * p.tiles_n, nsplit = ntiles - p.full_tiles;
     const int tile4 = tile_rows * tile_cols / 4;           // float4 per tile
@@ -313,6 +337,8 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
     // Ring depth: as many stages as fit (a stage is the A box + 16 KiB of W).  The kernel is bound by the weight stream,
     // and what keeps HBM busy is bytes in flight per SM: 6 stages (m = 128) .. 12 stages (m <= 16: 192 KiB of W in flight).
     const int stage_bytes = p.a_box_bytes + GM_B_BYTES;
+    // (Capping the ring at 110 KiB so that a CTA of the next call can move in beside this one was measured and is slower:
+    // m = 64 26.5 us against 23.9 us — what counts is the depth of the ring that is streaming.)
     q.stages = (GM_SMEM_MAX - 1024 - GM_BAR_BYTES) / stage_bytes;
     if (q.stages > GM_MAX_STAGES) q.stages = GM_MAX_STAGES;
     const int smem_bytes = gm_smem_bytes(q.stages, stage_bytes);
@@ -331,8 +357,17 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
         if (st != TRI_OK) return st;
         if (q.full_tiles == 0) grid = left * parts;
     }
-    gemm_1sm_kernel<<<grid, GM_THREADS, smem_bytes, s>>>(amap, wmap, q);
-    TRI_CUDA(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(GM_THREADS);
+    cfg.dynamicSmemBytes = smem_bytes;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_1sm_kernel, amap, wmap, q));
     if (q.parts > 1) return launch_splitk_reduce(q, GM_BM, GM_BN, false, s);
     return TRI_OK;
 }
@@ -359,7 +394,9 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     int st = ensure_init(&di);
     if (st != TRI_OK) return st;
 
-    const bool one_sm = m <= GM_BM;                           // a short A: 128 x 128 tiles, one CTA each (see the file header)
+    // a short A: 128 x 128 tiles, one CTA each (see the file header).  (128 < m <= 256 on this kernel, two row blocks per
+    // W panel, was measured: 36-37 us against 32-33 us for the pair kernel on m x 18944 x 3584.)
+    const bool one_sm = m <= GM_BM;
     const int rows_per_tile = one_sm ? GM_BM : 2 * GM_BM;
     const int cols_per_tile = one_sm ? GM_BN : 2 * GM_BN;
     cudaStream_t s = static_cast<cudaStream_t>(stream);

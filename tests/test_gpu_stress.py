@@ -92,3 +92,36 @@ def test_gemv_then_gemm_then_gemv_chain():
     within_bound(ys[0].cpu().numpy().view(np.uint16), x, wp, tri.TRI_W_NK)
     within_bound(cs[0].cpu().numpy().view(np.uint16), a, wp, tri.TRI_W_NK)
     assert all(torch.equal(y, ys[0]) for y in ys) and all(torch.equal(c, cs[0]) for c in cs)
+
+
+@pytest.mark.parametrize("m,n", [(16, 1024), (100, 640), (128, 2048)])
+def test_short_gemm_chain_orders_its_data_under_pdl(m, n):
+    """prefill_gemm for m <= 128 launches with programmatic stream serialization: call i + 1 starts (and prefetches W) while
+    call i drains, but may read A only after call i completed.  Here A of call i + 1 IS the output of call i (k = n, a
+    permutation-like W keeps the values bounded): C_{i+1} = C_i . W.  The chain without any host synchronisation must equal,
+    bit for bit, the same chain with a synchronisation after every call."""
+    k = n
+    a0 = normal_bf16(111, (m, k))
+    pi = np.random.default_rng(7).permutation(k)
+    wl = np.zeros((k, n), np.float32)
+    wl[pi, np.arange(n)] = 1.0
+    wl[(pi + 1) % k, np.arange(n)] = -0.5                       # two terms per output: not a pure copy
+    from synth_inputs import f32_to_bf16_bits
+    dw = dev(np.ascontiguousarray(f32_to_bf16_bits(wl).T))
+    depth = 12
+
+    def chain(sync):
+        bufs = [dev(a0)] + [torch.full((m, n), NAN16, dtype=torch.int16, device="cuda") for _ in range(depth)]
+        for i in range(depth):
+            tri.prefill_gemm(m, n, k, bufs[i], k, dw, k, tri.TRI_W_NK, bufs[i + 1], n)
+            if sync:
+                torch.cuda.synchronize()
+        torch.cuda.synchronize()
+        return bufs
+
+    ref, got = chain(True), chain(False)
+    first = ref[1].cpu().numpy().view(np.uint16)
+    within_bound(first, a0, np.ascontiguousarray(f32_to_bf16_bits(wl).T), tri.TRI_W_NK)
+    assert not torch.equal(ref[depth], ref[1])
+    for i in range(1, depth + 1):
+        assert torch.equal(got[i], ref[i]), f"link {i} of the unsynchronised chain differs"
