@@ -306,39 +306,58 @@ def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
     return out
 
 
+def time_gemm_pair(torch, tri, m, n, k, group=8):
+    """Device time per call (ms) of prefill_gemm and of torch.matmul (cuBLAS, context) on one m x n x k shape.  Weights
+    rotate over enough copies to exceed L2 (a model's next use of a matrix comes after all its other weights); calls are
+    timed in groups of `group` between one CUDA-event pair, median of 9 groups — an event pair around every single call
+    measures the host's launch rate, not the kernel, once a call is shorter than ~40 us — after a short rest, so that a
+    point does not inherit the power-capped clock of the one before it."""
+    copies = max(2, min(8, int(300e6 / (2.0 * n * k)) + 1))
+    a = torch.randn(m, k, device="cuda").bfloat16()
+    ws = [(torch.randn(n, k, device="cuda") * 0.02).bfloat16() for _ in range(copies)]
+    c = torch.empty(m, n, device="cuda", dtype=torch.bfloat16)
+
+    def med(fn):
+        torch.cuda.synchronize()
+        time.sleep(0.2)
+        for i in range(2 * group):
+            fn(ws[i % copies])
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(9)]
+        for x, y in ev:
+            x.record()
+            for i in range(group):
+                fn(ws[i % copies])
+            y.record()
+        torch.cuda.synchronize()
+        return sorted(x.elapsed_time(y) for x, y in ev)[4] / group
+
+    ours = med(lambda w: tri.prefill_gemm(m, n, k, a, k, w, k, tri.TRI_W_NK, c, n))
+    lib = med(lambda w: torch.matmul(a, w.T, out=c))
+    del a, ws, c
+    return ours, lib
+
+
+def gemm_point(series, m, n, k, ours, lib, peaks, **extra):
+    flop, nbytes = 2.0 * m * n * k, 2.0 * (m * k + n * k + m * n)
+    ai = flop / nbytes
+    roof = min(peaks["bf16_tflops"], ai * peaks["hbm_gbs"] / 1e3)
+    return dict({"kernel": "prefill_gemm", "series": series, "m": m, "n": n, "k": k, "ai": ai, "ms": ours, "tflops": flop / ours / 1e9,
+                 "gbs": nbytes / ours / 1e6, "roofline_tflops": roof, "frac": flop / ours / 1e9 / roof,
+                 "bound": "tensor" if roof == peaks["bf16_tflops"] else "hbm", "timing": "groups of 8 calls, rotating W copies",
+                 "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9}, **extra)
+
+
 def gemm_ai_series(torch, tri, peaks):
     """Row f4 (next): the paper's own microbenchmark form — a matmul whose A.I. is varied — on the
     tensor-core path: C[8192 x 8192] = A[8192 x K] W[K x 8192], bf16, K swept; A.I. = 2 m n K / (2 (m K + K n + m n)).
-    Roofline: min(measured cuBLAS burst, A.I. x measured HBM).  torch.matmul (cuBLAS) on the same operands is timed
-    beside it as context."""
+    Roofline: min(measured cuBLAS burst, A.I. x measured HBM copy rate).  The low-K points only write C: a write-only
+    stream reaches 3.6-3.9 TB/s on this part (torch fill), not the copy rate, so their `frac` has a ceiling
+    near 0.75.  torch.matmul (cuBLAS) on the same operands is timed beside it as context."""
     m = n = 8192
     out = []
     for k in (16, 64, 256, 1024, 4096):
-        a = (torch.randn(m, k, device="cuda")).bfloat16()
-        w = (torch.randn(n, k, device="cuda") * 0.02).bfloat16()
-        c = torch.empty(m, n, device="cuda", dtype=torch.bfloat16)
-
-        def med(fn):
-            for _ in range(20):                                           # the part idles between points: let the clocks come back
-                fn()
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(9)]
-            for x, y in ev:
-                x.record()
-                fn()
-                y.record()
-            torch.cuda.synchronize()
-            return sorted(x.elapsed_time(y) for x, y in ev)[4]
-
-        ours = med(lambda: tri.prefill_gemm(m, n, k, a, k, w, k, tri.TRI_W_NK, c, n))
-        lib = med(lambda: torch.matmul(a, w.T, out=c))
-        flop, nbytes = 2.0 * m * n * k, 2.0 * (m * k + n * k + m * n)
-        ai = flop / nbytes
-        roof = min(peaks["bf16_tflops"], ai * peaks["hbm_gbs"] / 1e3)
-        out.append({"kernel": "prefill_gemm", "series": "matmul-based A.I. sweep (PAPER.md line 92), 8192 x 8192 x K", "k": k, "ai": ai,
-                    "ms": ours, "tflops": flop / ours / 1e9, "gbs": nbytes / ours / 1e6, "roofline_tflops": roof,
-                    "frac": flop / ours / 1e9 / roof, "bound": "tensor" if roof == peaks["bf16_tflops"] else "hbm",
-                    "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9})
-        del a, w, c
+        ours, lib = time_gemm_pair(torch, tri, m, n, k)
+        out.append(gemm_point("matmul-based A.I. sweep (PAPER.md line 92), 8192 x 8192 x K", m, n, k, ours, lib, peaks))
     return out
 
 
@@ -347,31 +366,8 @@ def gemm_shape_series(torch, tri, peaks):
     roofline min(measured cuBLAS burst, A.I. x measured HBM) and torch.matmul (cuBLAS) on the same operands as context."""
     out = []
     for label, (m, n, k) in GEMM_SHAPES.items():
-        a = torch.randn(m, k, device="cuda").bfloat16()
-        w = (torch.randn(n, k, device="cuda") * 0.02).bfloat16()
-        c = torch.empty(m, n, device="cuda", dtype=torch.bfloat16)
-
-        def med(fn):
-            for _ in range(10):
-                fn()
-            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(11)]
-            for x, y in ev:
-                x.record()
-                fn()
-                y.record()
-            torch.cuda.synchronize()
-            return sorted(x.elapsed_time(y) for x, y in ev)[5]
-
-        ours = med(lambda: tri.prefill_gemm(m, n, k, a, k, w, k, tri.TRI_W_NK, c, n))
-        lib = med(lambda: torch.matmul(a, w.T, out=c))
-        flop, nbytes = 2.0 * m * n * k, 2.0 * (m * k + n * k + m * n)
-        ai = flop / nbytes
-        roof = min(peaks["bf16_tflops"], ai * peaks["hbm_gbs"] / 1e3)
-        out.append({"kernel": "prefill_gemm", "series": "Thinker-shaped GEMMs (SURVEY 8(f).4)", "label": label, "m": m, "n": n, "k": k,
-                    "ai": ai, "ms": ours, "tflops": flop / ours / 1e9, "gbs": nbytes / ours / 1e6, "roofline_tflops": roof,
-                    "frac": flop / ours / 1e9 / roof, "bound": "tensor" if roof == peaks["bf16_tflops"] else "hbm",
-                    "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9})
-        del a, w, c
+        ours, lib = time_gemm_pair(torch, tri, m, n, k)
+        out.append(gemm_point("Thinker-shaped GEMMs (SURVEY 8(f).4)", m, n, k, ours, lib, peaks, label=label))
     return out
 
 

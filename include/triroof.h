@@ -138,8 +138,9 @@ typedef struct {
     uint32_t sm_mhz, mem_mhz;   /* nvmlDeviceGetClockInfo(SM / MEM) */
     uint32_t temp_c;            /* GPU temperature */
     float power_w;              /* nvmlDeviceGetPowerUsage / 1000 */
-    uint64_t energy_mj;         /* nvmlDeviceGetTotalEnergyConsumption (0 if unsupported); inside a trace refreshed about
-                                 * every 100 ms and carried forward in between (the query takes 4-13 ms on B200) */
+    uint64_t energy_mj;         /* nvmlDeviceGetTotalEnergyConsumption (0 if unsupported); inside a trace polled by a thread
+                                 * of its own about every 100 ms and carried forward in between (the query takes 4-13 ms
+                                 * on B200, more than the 10 ms sampling period) */
     uint64_t clk_event_reasons; /* nvmlDeviceGetCurrentClocksEventReasons bitmask */
 } tri_sample;
 

@@ -504,7 +504,7 @@ static cudaError_t launch_gemv_rows(int m, const CUtensorMap &wmap, const CUtens
     return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
 }
 
-static int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
+int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
                      uint16_t *y, int64_t ldy, void *stream)
 {
     if (!x || !w || !y) return fail(TRI_ERR_INVALID_ARG, "x/w/y is NULL");

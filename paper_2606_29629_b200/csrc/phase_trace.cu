@@ -7,6 +7,7 @@
 #include "tri_internal.h"
 
 #include <time.h>
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstring>
@@ -43,8 +44,26 @@ struct Tracer {
     bool overflow = false;
     unsigned period_us = 10000;
     double t0 = 0.0;
-    uint64_t last_energy_mj = 0;
-    std::thread th;
+    std::atomic<uint64_t> energy_mj{0};
+    std::thread th, eth;
+
+    // The energy counter is the one slow NVML query (4-13 ms on B200, more while the driver is busy launching): it is polled
+    // by a thread of its own about every 100 ms and the sampler copies the last value, so that the clock / temperature /
+    // power samples keep the requested period whatever that query costs.
+    void run_energy()
+    {
+        const double step = period_us >= 100000 ? 1e-6 * period_us : 0.1;
+        double next = now_s();
+        while (!stop.load(std::memory_order_acquire)) {
+            unsigned long long e = 0;
+            if (api->total_energy && api->total_energy(dev, &e) == nvml::SUCCESS) energy_mj.store(e, std::memory_order_release);
+            next += step;
+            const double t = now_s();
+            if (next < t) next = t;
+            // sleep in slices of at most 20 ms so that stop() is not held up by a whole step
+            while (!stop.load(std::memory_order_acquire) && now_s() < next) sleep_until(std::min(next, now_s() + 0.02));
+        }
+    }
 
     void run()
     {
@@ -57,13 +76,8 @@ struct Tracer {
             }
             tri_sample s;
             memset(&s, 0, sizeof(s));
-            // the energy counter is the one slow NVML query (4-13 ms): read it about every 100 ms and carry the value
-            // forward in between, so that the clock / temperature / power samples keep the requested period
-            const size_t every = period_us >= 100000 ? 1 : (100000 + period_us - 1) / period_us;
-            const bool with_energy = (i % every) == 0;
-            s.energy_mj = last_energy_mj;
-            nvml::read_sample(api, dev, &s, with_energy);
-            last_energy_mj = s.energy_mj;
+            nvml::read_sample(api, dev, &s, false);
+            s.energy_mj = energy_mj.load(std::memory_order_acquire);
             s.t_s = now_s() - t0;                      // stamped after the reads: the values are at most this old
             s.phase = phase.load(std::memory_order_acquire);
             buf[i] = s;
@@ -130,7 +144,12 @@ int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t ca
     t->period_us = period_us;
     t->t0 = tri::now_s();
     tri::nvml::tracer_enter();                    // tri_shutdown() keeps NVML loaded while this sampler runs
+    {
+        unsigned long long e = 0;                 // the first sample already carries a counter value
+        if (a->total_energy && a->total_energy(h, &e) == tri::nvml::SUCCESS) t->energy_mj.store(e);
+    }
     t->th = std::thread([t] { t->run(); });
+    t->eth = std::thread([t] { t->run_energy(); });
     *handle = t;
     return TRI_OK;
 }
@@ -148,6 +167,7 @@ int phase_trace_stop(void *handle, size_t *n_samples)
     tri::Tracer *t = static_cast<tri::Tracer *>(handle);
     t->stop.store(true, std::memory_order_release);
     if (t->th.joinable()) t->th.join();
+    if (t->eth.joinable()) t->eth.join();
     tri::nvml::tracer_leave();
     if (n_samples) *n_samples = t->n.load();
     bool ovf = t->overflow;

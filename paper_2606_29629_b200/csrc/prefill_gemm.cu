@@ -5,7 +5,7 @@
 // one-CTA kernel used when A has at most 128 rows; m > 128 goes to the CTA-pair kernel of prefill_gemm_2sm.cu (256 x 256
 // pair tiles), which a short A would leave three quarters empty.
 //
-// One-CTA kernel (m <= 128: chunked-prefill tails, speculative / large-batch decode): weight-streaming bound, so the
+// One-CTA kernel (16 < m <= 128: chunked-prefill tails, speculative / large-batch decode; m <= 16 goes to the GEMV): weight-streaming bound, so the
 // tile is 128 x 128 — 148 tiles for n = 18944, one per SM — and when there are fewer tiles than SMs every tile is cut
 // along K into `parts` ranges (gemm_common.cuh next_work / splitk_*) so that all SMs pull on HBM.  Warp roles as in the
 // pair kernel: warp 0 TMA producer (A rows x 64 and W 128 x 64 per k-block into a 6- to 12-stage ring, 128-byte swizzle), warp 1
@@ -337,8 +337,12 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
     // Ring depth: as many stages as fit (a stage is the A box + 16 KiB of W).  The kernel is bound by the weight stream,
     // and what keeps HBM busy is bytes in flight per SM: 6 stages (m = 128) .. 12 stages (m <= 16: 192 KiB of W in flight).
     const int stage_bytes = p.a_box_bytes + GM_B_BYTES;
-    // (Capping the ring at 110 KiB so that a CTA of the next call can move in beside this one was measured and is slower:
-    // m = 64 26.5 us against 23.9 us — what counts is the depth of the ring that is streaming.)
+    // (Capping the ring at 112 KiB so that a CTA of the next call moves in beside this one was measured: m = 16 23.8 us
+    // against 23.7 us, m = 64 26.6 against 23.9.  In-kernel %globaltimer stamps show why it cannot win: the early CTA fills
+    // its ring with W and then sits in griddepcontrol.wait until the whole grid before it has completed, so what a call
+    // costs is (1 - ring / panel) of the stream plus the same fixed part either way — A's L2 latency after the wait 0.9 us,
+    // last MMA to exit 1.2 us, grid completion to the dependents' release 1.1 us, 3-5 us of skew between the SMs — and a
+    // deeper ring in ONE CTA prefetches as much as two shallow ones.)
     q.stages = (GM_SMEM_MAX - 1024 - GM_BAR_BYTES) / stage_bytes;
     if (q.stages > GM_MAX_STAGES) q.stages = GM_MAX_STAGES;
     const int smem_bytes = gm_smem_bytes(q.stages, stage_bytes);
@@ -390,6 +394,12 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
         const uintptr_t w0 = (uintptr_t)w, w1 = w0 + ((wrows - 1) * (size_t)ldw + wcols) * 2;
         if ((c0 < a1 && a0 < c1) || (c0 < w1 && w0 < c1)) return fail(TRI_ERR_INVALID_ARG, "c aliases an input");
     }
+    // At most 16 rows: the contraction is a weight stream with a sliver of arithmetic, and the streaming GEMV (two CTAs per
+    // SM, warp-level MMA, no TMEM set-up, no epilogue to speak of) does it in 21.5 us back to back on 16 x 18944 x 3584
+    // where the 128-row tcgen05 tile below needs 23.7 us.  Same definition, same rounding; every argument rule of this
+    // entry point is at least as strict as the GEMV's.
+    if (m <= 16) return gemv_impl(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream);
+
     const DeviceInfo *di = nullptr;
     int st = ensure_init(&di);
     if (st != TRI_OK) return st;

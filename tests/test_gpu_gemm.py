@@ -176,9 +176,10 @@ def test_down_projection_sampled_rows(layout):
 
 
 @pytest.mark.parametrize("layout", LAYOUTS)
-@pytest.mark.parametrize("m", [16, 64, 128])
+@pytest.mark.parametrize("m", [16, 24, 64, 128])
 def test_short_a_up_projection(layout, m):
-    """m <= 128 runs the one-CTA kernel (128 x 128 tiles): the config-4 weights with a short A; 148 tiles, no split."""
+    """16 < m <= 128 runs the one-CTA kernel (128 x 128 tiles; m = 24: a 24-row A box), m <= 16 is handed to the streaming
+    GEMV: the config-4 weights with a short A; 148 tiles, no split."""
     k, n = 3584, 18944
     a = normal_bf16(3, (m, k), 1.0, stream=4)
     w = normal_bf16(3, (k, n), 0.02, stream=1)

@@ -59,7 +59,7 @@ def test_phase_trace_driver_short():
     names = [s["phase_name"] for s in summ]
     assert names == (["prefill", "decode", "idle"] * 2)[:len(names)] and len(names) >= 5   # phases overrun by a launch or two:
                                                                                          # the last idle may be cut at total_s
-    assert 0.9 * 2.0 / 0.010 <= len(samples) <= 230           # the 10 ms period of config 5 is held (energy is refreshed every 100 ms)
+    assert 0.93 * 2.0 / 0.010 <= len(samples) <= 230          # the 10 ms period of config 5 is held (the slow energy query has a thread of its own)
     for i, s in enumerate(summ):
         assert s["t_end_s"] > s["t_begin_s"]
         if s["phase_name"] == "idle":
@@ -69,7 +69,7 @@ def test_phase_trace_driver_short():
         else:
             assert s["launches"] > 10 and s["gpu_ms"] > 300
             assert s["energy_j"] > 0 and s["j_per_flop"] > 0 and s["j_per_token"] > 0
-            assert s["n_samples"] >= 0.8 * 40 and s["sm_mhz_mean"] > 0      # 0.4 s / 10 ms = 40 nominal
+            assert s["n_samples"] >= 0.85 * 40 and s["sm_mhz_mean"] > 0     # 0.4 s / 10 ms = 40 nominal
             per = 2.0 * (pm * pn * pk if s["phase_name"] == "prefill" else dm * dn * dk)
             assert abs(s["flop"] - per * s["launches"]) < 1e-3 * s["flop"]
     # the sampler tagged samples with the phase the driver was in
