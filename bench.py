@@ -409,7 +409,14 @@ def compact_line(full):
                         short(pj * 1e12 if pj else None, 2)])
     if len(sus) == len(pts) and sus:
         out["sustained"] = sus
-        out["sustained_cols"] = "in the order of fracs: frac at clock, SM MHz, W, pJ/FLOP"
+        out["sustained_cols"] = "order of fracs: frac at clock, SM MHz, W, pJ/FLOP"
+    # the extra FMA series of the sustained pass (between the powers of two around the ridge; the paper's own A.I. set):
+    # fraction of the roofline at the recorded clock, keyed by k
+    xs = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "fma_chain" and q.get("frac_sustained_at_clock") is not None]
+    for key, tag in (("ridge", "ridge"), ("paper_ai", "paper A.I.")):
+        sel = {f"k{q['k']}": round(q["frac_sustained_at_clock"], 2) for q in xs if str(q.get("series", "")).startswith(tag)}
+        if sel:
+            out[key] = sel
     gm = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "prefill_gemm" and q.get("label")]
     if gm:
         out["gemm_shapes"] = {q["label"]: round(q["frac"], 3) for q in gm}
