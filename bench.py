@@ -347,6 +347,48 @@ def gemm_point(series, m, n, k, ours, lib, peaks, **extra):
                  "cublas_ms": lib, "cublas_tflops": flop / lib / 1e9}, **extra)
 
 
+def controller_preview(tri, fit, pf, peaks, fma_pts, points, eps=0.05):
+    """Row f3 end to end on this run's own data (Eq. 5 and Eq. 6): the phase A.I. of
+    Eq. 5 from the measured kernel durations, and the clock Eq. 6 selects (the library's binary search, tri_solve_clock) on
+    the fitted throughput model, per A.I. point, with f_limit = the auto-boost clock this run recorded at that point.
+    P_idle(f) and P_dyn(f) exist on this pool only at the boost ceiling (no locked-clock columns), so the power tables are
+    that one fitted pair scaled LINEARLY in f — an assumption, stated in the output; Eq. 6's answer depends on them only
+    through their monotonicity (the paper's own premise, line 186), i.e. it is the lowest clock that keeps the throughput
+    within eps.  Nothing is actuated: clock locking is not used on this pool (R17)."""
+    fmax = peaks["sm_max_mhz"]
+    clocks = [float(f) for f in range(1005, int(fmax) + 1, 15)]       # a 15 MHz grid up to the boost ceiling, the step NVML reports on B200
+    if clocks[-1] != fmax:
+        clocks.append(fmax)
+    mdl = tri.Model(fit["eta"], fit["beta"], fit["omega"], fit["gamma"], p_tdp=1000.0, f_mhz=clocks,
+                    p_idle_w=[pf["p_idle_w"] * f / fmax for f in clocks], p_dyn_w=[pf["p_dyn_w"] * f / fmax for f in clocks])
+    rows = []
+    for pt in fma_pts:
+        f_limit = float(pt["sustained"]["sm_mhz"])
+        try:
+            mdl.validate(pt["ai"])
+            idx, feasible = mdl.solve_clock(pt["ai"], f_limit, eps)
+            rows.append({"ai": pt["ai"], "f_autoboost_mhz": f_limit, "f_selected_mhz": clocks[idx], "feasible": feasible,
+                         "theta_ratio": mdl.theta(pt["ai"], clocks[idx]) / mdl.theta(pt["ai"], fmax),
+                         "p_model_ratio": mdl.power(pt["ai"], idx) / mdl.power(pt["ai"], len(clocks) - 1)})
+        except tri.TriError as e:
+            rows.append({"ai": pt["ai"], "error": str(e)})
+    # Eq. 5 over the kernels of the timed step: the whole FMA sweep as one "phase", and the decode phase (8 GEMVs)
+    sweep = [pt for pt in points if pt["kernel"] == "fma_chain"]
+    gemv = next(pt for pt in points if pt["kernel"] == "decode_gemv")
+    ai_sweep = tri.tri_phase_ai([pt["ms"] for pt in sweep], [pt["ai"] for pt in sweep])
+    ai_decode = tri.tri_phase_ai([gemv["ms"]] * GEMV_COPIES, [gemv["ai"]] * GEMV_COPIES)
+    dec = {}
+    try:                                                               # the decode phase on the CUDA-core throughput model
+        idx, feasible = mdl.solve_clock(ai_decode, float((gemv.get("sustained") or {}).get("sm_mhz") or fmax), eps)
+        dec = {"f_selected_mhz": clocks[idx], "feasible": feasible, "f_autoboost_mhz": (gemv.get("sustained") or {}).get("sm_mhz")}
+    except tri.TriError as e:
+        dec = {"error": str(e)}
+    return {"eps": eps, "clock_grid_mhz": [clocks[0], clocks[-1], 15], "eq5_phase_ai": {"fma_sweep": ai_sweep, "decode": ai_decode},
+            "eq6_decode_phase": dec, "eq6_per_point": rows,
+            "assumption": "P_idle(f), P_dyn(f) = the boost-ceiling fit scaled linearly in f (no locked-clock data on this pool); "
+                          "Eq. 6 then returns the lowest clock within eps of the throughput at f_max; nothing is actuated"}
+
+
 def gemm_ai_series(torch, tri, peaks):
     """Row f4 (next): the paper's own microbenchmark form — a matmul whose A.I. is varied — on the
     tensor-core path: C[8192 x 8192] = A[8192 x K] W[K x 8192], bf16, K swept; A.I. = 2 m n K / (2 (m K + K n + m n)).
@@ -420,6 +462,9 @@ def compact_line(full):
     gm = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "prefill_gemm" and q.get("label")]
     if gm:
         out["gemm_shapes"] = {q["label"]: round(q["frac"], 3) for q in gm}
+    cp = ((full.get("model_fit") or {}).get("controller_preview") or {}).get("eq6_decode_phase") or {}
+    if cp.get("f_selected_mhz"):                                       # Eq. 6 on the fitted model, decode phase: [selected, auto-boost] MHz
+        out["eq6_decode_mhz"] = [int(cp["f_selected_mhz"]), int(cp.get("f_autoboost_mhz") or 0)]
     if full.get("energy"):
         out["j_per_flop"] = sig(full["energy"].get("j_per_flop"), 3)
     out["detail"] = DETAIL_FILE
@@ -598,6 +643,7 @@ def run_ours(args):
                                            peaks["sm_max_mhz"], 2.0, 950.0)
                     model_fit["power_at_max_clock"] = dict(pf, f_mhz=peaks["sm_max_mhz"],
                                                            source="PAPER.md Eq. 2-3 via tri_fit_power on the points at the boost ceiling, below the power cap")
+                    model_fit["controller_preview"] = controller_preview(tri, fit, pf, peaks, fma_pts, points)
                 except tri.TriError as e:
                     model_fit["power_at_max_clock"] = {"error": str(e)}
             except tri.TriError as e:

@@ -84,3 +84,36 @@ def test_reference_arm_last_line_parses():
     d = json.loads(last)
     assert d["impl"] == "reference" and d["value"] > 0 and d["unit"] == bench.UNIT and d["metric"] == bench.METRIC
     assert d["config"] == bench.workload_config(1)
+
+
+def test_controller_preview_on_a_synthetic_sweep():
+    """bench.controller_preview (row f3 end to end: Eq. 5 + Eq. 6 on the fitted model) on points generated from a planted Eq. 4
+    model: memory-bound points get a clock well below the boost ceiling with the throughput within eps, compute-bound points
+    keep (1 - eps) of f_max, and Eq. 5 of equal-A.I. kernels is that A.I."""
+    import paper_2606_29629_b200 as tri
+    eta, beta, omega, gamma, fmax = 0.0377, 6.87, 0.7, 0.0, 1965.0
+    peaks = {"sm_max_mhz": fmax}
+
+    def theta(ai, f):
+        return min(eta * f * ai / (ai + omega), beta * ai)
+    pts = [{"kernel": "fma_chain", "k": k, "ai": k / 4.0, "ms": 2.0 * k * bench.N_FMA / theta(k / 4.0, fmax) / 1e9,
+            "sustained": {"sm_mhz": 1600.0 if k == 32 else fmax, "tflops_sustained": theta(k / 4.0, fmax)}} for k in bench.KS]
+    gemv = {"kernel": "decode_gemv", "ai": 7.98, "ms": 0.0215, "sustained": {"sm_mhz": 1650.0}}
+    out = bench.controller_preview(tri, {"eta": eta, "beta": beta, "omega": omega, "gamma": gamma}, {"p_idle_w": 500.0, "p_dyn_w": 900.0},
+                                   peaks, pts, pts + [gemv])
+    assert abs(out["eq5_phase_ai"]["decode"] - 7.98) < 1e-12
+    total = sum(p["ms"] for p in pts)
+    assert abs(out["eq5_phase_ai"]["fma_sweep"] - sum(p["ms"] * p["ai"] for p in pts) / total) < 1e-9
+    rows = {r["ai"]: r for r in out["eq6_per_point"]}
+    assert len(rows) == len(bench.KS) and all("error" not in r for r in rows.values())
+    for ai, r in rows.items():
+        assert r["f_selected_mhz"] <= r["f_autoboost_mhz"] + 1e-9
+        if r["feasible"]:
+            assert r["theta_ratio"] >= 0.95 - 1e-12
+    assert rows[0.25]["f_selected_mhz"] == 1005.0 and rows[0.25]["feasible"]          # far memory-bound: the lowest clock suffices
+    assert rows[1024.0]["f_selected_mhz"] >= 0.95 * fmax - 15 and rows[1024.0]["feasible"]   # compute-bound: theta ~ f
+    assert rows[1024.0]["p_model_ratio"] < 1.0 < 1.0 + rows[0.25]["p_model_ratio"]
+    assert not rows[8.0]["feasible"] or rows[8.0]["f_selected_mhz"] <= 1600.0        # f_limit = the auto-boost clock of that point
+    d = out["eq6_decode_phase"]
+    assert d["feasible"] and 1005.0 <= d["f_selected_mhz"] <= 1650.0
+    json.dumps(out)
