@@ -125,3 +125,33 @@ def test_short_gemm_chain_orders_its_data_under_pdl(m, n):
     assert not torch.equal(ref[depth], ref[1])
     for i in range(1, depth + 1):
         assert torch.equal(got[i], ref[i]), f"link {i} of the unsynchronised chain differs"
+
+
+def test_shutdown_then_reuse():
+    """tri_shutdown() frees what the library allocated (split-K workspaces, the clock-probe scratch, NVML) and the next call
+    re-initialises lazily: the same calls give the same bits before and after, and NVML sampling comes back."""
+    m, n, k = 64, 392, 2048                                  # one-CTA kernel, 4 tiles cut along K: needs the workspace
+    a, w = normal_bf16(121, (m, k)), normal_bf16(122, (k, n), 0.05)
+    wp = np.ascontiguousarray(w.T)
+    da, dw = dev(a), dev(wp)
+    x = normal_bf16(123, (8, k))
+    dx = dev(x)
+
+    def once():
+        c = torch.full((m, n), NAN16, dtype=torch.int16, device="cuda")
+        y = torch.full((8, n), NAN16, dtype=torch.int16, device="cuda")
+        tri.prefill_gemm(m, n, k, da, k, dw, k, tri.TRI_W_NK, c, n)
+        tri.decode_gemv(8, n, k, dx, k, dw, k, tri.TRI_W_NK, y, n)
+        mhz = tri.tri_sm_clock_mhz(200)
+        torch.cuda.synchronize()
+        return c, y, mhz
+
+    c0, y0, mhz0 = once()
+    within_bound(c0.cpu().numpy().view(np.uint16), a, wp, tri.TRI_W_NK)
+    tri.tri_shutdown()
+    tri.tri_shutdown()                                       # idempotent
+    c1, y1, mhz1 = once()
+    assert torch.equal(c0, c1) and torch.equal(y0, y1)
+    assert 500 < mhz0 < 2200 and 500 < mhz1 < 2200
+    assert tri.tri_nvml_sample(0)["sm_mhz"] > 0
+    assert tri.sm_count() == 148 or tri.sm_count() > 0
