@@ -117,12 +117,16 @@ static int run(unsigned k, float a, float b, size_t n, const float *in, float *o
     int st = ensure_init(nullptr);
     if (st != TRI_OK) return st;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    // float4 loads in flight per thread (= 4 x VEC chains), chosen by measurement on B200 (N = 2^28): the memory-bound
-    // end likes many small blocks (VEC 2: 6.85 TB/s), the ridge needs both the load queue and the FP32 pipe full
-    // (VEC 4 at k = 32, VEC 8 from k = 40: 1.04 of the HBM roof there instead of 0.96, 0.95-0.98 of the ALU roof from k = 48
-    // instead of 0.90-0.96; VEC 16 is no better), the far compute-bound end
-    // is indifferent (VEC 2: 0.998).
-    const int vec = k <= 24 ? 2 : k <= 35 ? 4 : k < 2048 ? 8 : 2;
+    // float4 loads in flight per thread (= 4 x VEC chains), chosen by measurement on B200 (N = 2^28) in BOTH regimes the
+    // bench reports: a single launch at the boost clock, and a seconds-long loop, where the 1000 W cap pulls the clock to
+    // ~1.5 GHz and moves the ridge down to k ~ 36.  Fraction of min(A.I. x HBM, ALU at the recorded clock), burst / sustained:
+    //   k = 16: VEC 2 1.04 / 1.07, VEC 4 1.03 / 1.04          k = 24: VEC 2 1.06 / 0.97, VEC 4 1.04 / 1.04
+    //   k = 28: VEC 4 1.03 / 0.98, VEC 8 1.03 / 1.03          k = 32: VEC 4 1.04 / 0.93, VEC 8 1.03 / 0.995
+    //   k = 40: VEC 4 0.95 / 0.88, VEC 8 1.04 / 0.95          k = 64: VEC 4 - / 0.94,  VEC 8 0.965 / 0.97
+    // More chains per thread mean fewer address / loop instructions per element: under the cap the kernel then draws less
+    // power per byte, and at k = 32 it is faster at 1462 MHz (VEC 8) than at 1545 MHz (VEC 4).  The far compute-bound end is
+    // indifferent (VEC 2: 0.998); VEC 16 is no better anywhere.
+    const int vec = k <= 16 ? 2 : k <= 24 ? 4 : k < 2048 ? 8 : 2;
     cudaError_t e;
     switch (vec) {
         case 2: e = launch<2>(in, out, n, k, a, b, s); break;
