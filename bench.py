@@ -560,19 +560,22 @@ def run_ours(args):
         points.append({"kernel": "fma_chain", "k": k, "ai": k / 4.0, "ms": ms, "gbs": gbs, "tflops": tf,
                        "bound": "hbm" if k / 4.0 * peaks["hbm_gbs"] / 1e3 < alu_peak else "alu",
                        "roofline_tflops": roof, "frac": tf / roof, "ms_min": min(per[f"fma_k{k}"]),
-                       "frac_vs_nominal": tf / min(alu_peak, k / 4.0 * NOMINAL_HBM_GBS / 1e3)})
+                       "frac_vs_nominal": tf / min(alu_peak, k / 4.0 * NOMINAL_HBM_GBS / 1e3), "algorithmic_bytes": 8.0 * N_FMA,
+                       "traffic": ncu_traffic_bytes("fma_chain", column=KS.index(k))})
     ms = statistics.median(per["gemv"]) / GEMV_COPIES
     gv_gbs = gemm_bytes(GEMV_SHAPE) / ms / 1e6
     points.append({"kernel": "decode_gemv", "ai": gemm_flop(GEMV_SHAPE) / gemm_bytes(GEMV_SHAPE), "ms": ms, "gbs": gv_gbs,
                    "tflops": gemm_flop(GEMV_SHAPE) / ms / 1e9, "bound": "hbm", "roofline_gbs": peaks["hbm_gbs"],
                    "frac": gv_gbs / peaks["hbm_gbs"], "ms_min": min(per["gemv"]) / GEMV_COPIES,
-                   "frac_vs_nominal": gv_gbs / NOMINAL_HBM_GBS})
+                   "frac_vs_nominal": gv_gbs / NOMINAL_HBM_GBS, "algorithmic_bytes": gemm_bytes(GEMV_SHAPE),
+                   "traffic": ncu_traffic_bytes("decode_gemv", column=0)})
     ms = statistics.median(per["gemm"])
     gm_tf = gemm_flop(GEMM_SHAPE) / ms / 1e9
     points.append({"kernel": "prefill_gemm", "ai": gemm_flop(GEMM_SHAPE) / gemm_bytes(GEMM_SHAPE), "ms": ms,
                    "gbs": gemm_bytes(GEMM_SHAPE) / ms / 1e6, "tflops": gm_tf, "bound": "tensor",
                    "roofline_tflops": peaks["bf16_tflops"], "frac": gm_tf / peaks["bf16_tflops"], "ms_min": min(per["gemm"]),
-                   "frac_vs_nominal": gm_tf / NOMINAL_BF16_TFLOPS})
+                   "frac_vs_nominal": gm_tf / NOMINAL_BF16_TFLOPS, "algorithmic_bytes": gemm_bytes(GEMM_SHAPE),
+                   "traffic": ncu_traffic_bytes("prefill_gemm", column=0)})
 
     # ---- per-point sustained pass: clock, temperature, power, J/op per A.I. point and per phase kernel ----
     extra_points, model_fit = [], None
