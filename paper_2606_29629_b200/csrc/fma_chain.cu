@@ -3,7 +3,7 @@
 //
 //   out[i] = chain_k(in[i]),  chain: y <- fmaf(a, y, b) repeated k times, fp32 RN, fused.
 //
-// Layout: a tile is THREADS * VEC float4 (coalesced: float4 j of thread t sits at tile + j*THREADS + t).
+// Layout: a tile is FMA_THREADS * VEC float4 (coalesced: float4 j of thread t sits at tile + j*FMA_THREADS + t).
 // Every thread carries VEC*4 independent chains (VEC*2 packed FFMA2 chains), which hides the FFMA
 // latency at the compute end; at the memory end all VEC 128-bit loads are issued before the first
 // FMA.  The k loop is a runtime loop (k is arbitrary, not a power of two) unrolled by 8 with a
@@ -16,7 +16,6 @@
 
 namespace tri {
 
-constexpr int FMA_THREADS = 256;
 
 __device__ __forceinline__ float4 ld_stream(const float4 *p)
 {
@@ -49,7 +48,7 @@ __device__ __forceinline__ void chain_steps(float2 (&y)[NPAIR], unsigned k, floa
 }
 
 // n4 = number of whole float4 groups; `tail` (< 4) scalars follow them and are done by block 0.
-template <int VEC>
+template <int VEC, int FMA_THREADS>
 __global__ void __launch_bounds__(FMA_THREADS)
 fma_chain_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n4, unsigned tail, unsigned k, float a, float b)
 {
@@ -91,7 +90,7 @@ fma_chain_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n
     }
 }
 
-template <int VEC>
+template <int VEC, int FMA_THREADS>
 static cudaError_t launch(const float *in, float *out, size_t n, unsigned k, float a, float b, cudaStream_t s)
 {
     size_t n4 = n / 4;
@@ -99,7 +98,7 @@ static cudaError_t launch(const float *in, float *out, size_t n, unsigned k, flo
     size_t per = (size_t)FMA_THREADS * VEC;
     size_t blocks = (n4 + per - 1) / per;
     if (blocks == 0) blocks = 1;   // tail only
-    fma_chain_kernel<VEC><<<(unsigned)blocks, FMA_THREADS, 0, s>>>(in, out, n4, tail, k, a, b);
+    fma_chain_kernel<VEC, FMA_THREADS><<<(unsigned)blocks, FMA_THREADS, 0, s>>>(in, out, n4, tail, k, a, b);
     return cudaGetLastError();
 }
 
@@ -127,11 +126,16 @@ static int run(unsigned k, float a, float b, size_t n, const float *in, float *o
     // power per byte, and at k = 32 it is faster at 1462 MHz (VEC 8) than at 1545 MHz (VEC 4).  The far compute-bound end is
     // indifferent (VEC 2: 0.998); VEC 16 is no better anywhere.
     const int vec = k <= 16 ? 2 : k <= 24 ? 4 : k < 2048 ? 8 : 2;
+    // Block size: 256 threads; 128 for the compute-leaning VEC 8 range (k >= 48), where a launch is a few dozen waves of long
+    // blocks and the last, partly filled wave costs one block's duration: halving the block halves it (sustained, fraction of
+    // the roofline at the recorded clock: k = 64 0.969 -> 0.975, k = 128 0.981 -> 0.984, k = 256 0.987 -> 0.990; at k = 32
+    // the smaller block is slower in a burst, 1.01 against 1.03).  256-bit accesses (ld / st.global.v8.f32, SASS LDG.E.256)
+    // were measured at k <= 32 and change nothing: 6.83-6.90 TB/s either way, the stream is HBM-bound.
     cudaError_t e;
     switch (vec) {
-        case 2: e = launch<2>(in, out, n, k, a, b, s); break;
-        case 8: e = launch<8>(in, out, n, k, a, b, s); break;
-        default: e = launch<4>(in, out, n, k, a, b, s); break;
+        case 2: e = launch<2, 256>(in, out, n, k, a, b, s); break;
+        case 8: e = k >= 48 ? launch<8, 128>(in, out, n, k, a, b, s) : launch<8, 256>(in, out, n, k, a, b, s); break;
+        default: e = launch<4, 256>(in, out, n, k, a, b, s); break;
     }
     if (e != cudaSuccess) return fail(TRI_ERR_CUDA, "fma_chain launch: %s", cudaGetErrorString(e));
     return TRI_OK;
