@@ -157,6 +157,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         const uint32_t stage0 = outbuf + ew * 8192;
         uint32_t tcount = 0, sb = 0;
         if (lane == 0) ptx::prefetch_tmap(&cmap);
+        const uint64_t pol_c = ptx::policy_evict_first();
         GemmWork wk;
         for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i, ++tcount) {
             int tm, tn;
@@ -220,7 +221,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
                 ptx::fence_proxy_async_smem();                        // generic-proxy writes visible to the TMA engine
                 __syncwarp();
                 if (lane == 0) {
-                    if (row0 < p.m && tn * G2_BN + g * 64 < (p.n & ~7)) ptx::tma_store_2d(&cmap, buf, tn * G2_BN + g * 64, row0);
+                    if (row0 < p.m && tn * G2_BN + g * 64 < (p.n & ~7)) ptx::tma_store_2d_hint(&cmap, buf, tn * G2_BN + g * 64, row0, pol_c);
                     // one bulk group per buffer toggle, also when nothing was stored (an empty group is legal): wait_read<1>
                     // above counts groups, and must mean "the store before the previous one" for the buffer it guards
                     ptx::tma_store_commit();
