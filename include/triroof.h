@@ -22,6 +22,10 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream). Compute calls
  *     validate their arguments on the host BEFORE any CUDA call, enqueue their kernel(s) on
  *     `stream` and return; asynchronous faults surface at the caller's next synchronisation.
+ *   - CUDA graphs: the compute calls (roofline_run, decode_gemv, prefill_gemm) enqueue kernels only, so a sequence of
+ *     them can be captured in a CUDA graph once each distinct call has run once on the capture stream (a prefill_gemm
+ *     shape that is split along k allocates that stream's fp32 workspace on first use, which capture does not allow);
+ *     replays give the bits of the eager calls (tested).
  *   - There is no CPU fallback: a device that is not compute capability 10.x yields TRI_ERR_ARCH.
  *   - bf16 values are passed as raw uint16_t bit patterns.
  */

@@ -155,3 +155,43 @@ def test_shutdown_then_reuse():
     assert 500 < mhz0 < 2200 and 500 < mhz1 < 2200
     assert tri.tri_nvml_sample(0)["sm_mhz"] > 0
     assert tri.sm_count() == 148 or tri.sm_count() > 0
+
+
+def test_calls_are_capturable_in_a_cuda_graph():
+    """Every compute call enqueues kernels only (tensor maps are host-encoded kernel parameters, the split-K workspace of a
+    stream is allocated on that stream's first split call), so after one warm-up step on the capture stream a step can be
+    captured in a CUDA graph — programmatic dependent launches, the reduction kernel and the K-split clusters included — and
+    the replay gives the bits of the eager step."""
+    n_f = (1 << 20) + 3
+    x = torch.from_numpy(np.random.default_rng(3).uniform(-1, 1, n_f).astype(np.float32)).cuda()
+    y = torch.empty_like(x)
+    gx, gw = dev(normal_bf16(131, (8, 3584))), dev(np.ascontiguousarray(normal_bf16(132, (3584, 520), 0.05).T))   # K-split cluster launch
+    gy = torch.empty((8, 520), dtype=torch.int16, device="cuda")
+    pa, pw = dev(normal_bf16(133, (300, 2048))), dev(np.ascontiguousarray(normal_bf16(134, (2048, 704), 0.05).T))  # pair kernel, tail split
+    pc = torch.empty((300, 704), dtype=torch.int16, device="cuda")
+    sa, sw = dev(normal_bf16(135, (64, 2048))), dev(np.ascontiguousarray(normal_bf16(136, (2048, 392), 0.05).T))   # one-CTA kernel, split, PDL
+    sc = torch.empty((64, 392), dtype=torch.int16, device="cuda")
+
+    def step():
+        tri.roofline_run(6.0, n_f, x, y)
+        tri.prefill_gemm(300, 704, 2048, pa, 2048, pw, 2048, tri.TRI_W_NK, pc, 704)
+        tri.prefill_gemm(64, 392, 2048, sa, 2048, sw, 2048, tri.TRI_W_NK, sc, 392)
+        for _ in range(3):
+            tri.decode_gemv(8, 520, 3584, gx, 3584, gw, 3584, tri.TRI_W_NK, gy, 520)
+
+    outs = (y, pc, sc, gy)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        step()
+        s.synchronize()
+        ref = [t.clone() for t in outs]
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            step()
+        for t in outs:
+            t.zero_()
+        g.replay()
+        g.replay()
+        s.synchronize()
+    for a, b in zip(ref, outs):
+        assert torch.equal(a, b)
