@@ -580,6 +580,12 @@ def run_ours(args):
                    "frac_vs_nominal": gm_tf / NOMINAL_BF16_TFLOPS, "algorithmic_bytes": gemm_bytes(GEMM_SHAPE),
                    "traffic": ncu_traffic_bytes("prefill_gemm", column=0)})
 
+    # the paper takes a kernel's A.I. from Nsight Compute: FLOP over the DRAM bytes ncu counted for the launch
+    for pt in points:
+        if pt.get("traffic"):
+            flop = fma_flop(pt["k"]) if pt["kernel"] == "fma_chain" else gemm_flop(GEMV_SHAPE if pt["kernel"] == "decode_gemv" else GEMM_SHAPE)
+            pt["ai_from_ncu_traffic"] = flop / pt["traffic"]
+
     # ---- per-point sustained pass: clock, temperature, power, J/op per A.I. point and per phase kernel ----
     extra_points, model_fit = [], None
     if args.char_seconds > 0 and world == 1:
