@@ -781,7 +781,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--char-seconds", type=float, default=0.5,
+    ap.add_argument("--char-seconds", type=float, default=1.0,
                     help="seconds of sustained looping per A.I. point for clock / temperature / J-per-op (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
