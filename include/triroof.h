@@ -124,6 +124,7 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
  * a, w, c 16-byte aligned.  Ragged m, n, k tiles are handled inside (TMA zero fill, clipped stores).
  * Outputs must not alias inputs.  Asynchronous: one kernel on `stream` (two when the shape is split along k: the
  * second adds the fp32 partial tiles in a fixed order).
+ * m <= 32 is computed by decode_gemv's streaming kernels (same definition and rounding).
  * For m <= 128 the kernel is launched with programmatic stream serialization, like decode_gemv: it prefetches W
  * (model state) while the kernel before it on `stream` drains, and reads A / writes C only after that kernel has
  * completed.  W must therefore not be an output of the immediately preceding prefill_gemm / decode_gemv call on

@@ -27,9 +27,10 @@
 //       - TRI_W_KN (slot row = k, 128 B = 64 columns n): lane (c = lane & 7, q = lane >> 3) of warp w owns the 8
 //         columns of chunk c and the k-rows 16w + 4q .. + 3; 16 partial sums per output.
 //
-// (2) 5 <= m <= 16: the warp-level tensor-core instruction  mma.sync.m16n8k16 (bf16 in, fp32 accumulate; SASS HMMA)
-//     with the WEIGHT tile as the 16-row operand and the batch as n = 8 (one tile for m <= 8, two for m <= 16): zero
-//     padding waste at m = 8, and W is still read once at m = 16.  Why not CUDA cores here (DESIGN.md §5.2 has the
+// (2) 5 <= m <= 32: the warp-level tensor-core instruction  mma.sync.m16n8k16 (bf16 in, fp32 accumulate; SASS HMMA)
+//     with the WEIGHT tile as the 16-row operand and the batch as n = 8 (one tile for m <= 8, two for m <= 16, four for
+//     m <= 32 — the last only through prefill_gemm, decode_gemv's ABI stops at 16): zero padding waste at m = 8, and W is
+//     still read once at m = 32.  Why not CUDA cores here (DESIGN.md §5.2 has the
 //     numbers): m FMAs per weight are 14.6 us of FMA-pipe time at m = 8 and 1965 MHz (17 us at the ~1.7 GHz the part
 //     holds under its power cap) inside a 20.8 us HBM budget, and 29 us at m = 16 — the round-1 FFMA2 / FHFMA kernels
 //     stopped at 24.8 us back to back and 26.9 us inside the bench step (0.77 of the roofline) with the FMA pipe 60 %
@@ -53,6 +54,7 @@ constexpr int GV_STAGE_K = 64;           // k-values per stage
 constexpr int GV_W_BYTES = GV_STAGE_K * GV_COLS * 2;  // 8 KiB
 constexpr int GV_XROW_BYTES = GV_STAGE_K * 2;         // 128 B: one batch row of a stage
 constexpr int GV_MAX_SLOTS = 10;
+constexpr int GV_MAX_ROWS = 32;          // rows the kernels take (decode_gemv's ABI stops at 16; prefill_gemm hands over up to 32)
 constexpr int GV_BAR_BYTES = 2 * 8 * GV_MAX_SLOTS;    // full[], empty[]
 constexpr int GV_RED_STRIDE = 4 * GV_COLS + 16;       // FHFMA path: floats per partial-sum set; +16 keeps the two half-warps on different banks
 
@@ -364,7 +366,7 @@ gemv_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant__ CU
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
-// (2) Warp-MMA path, 5 <= m <= 16.  NT: batch tiles of 8 rows (1 or 2).
+// (2) Warp-MMA path, 5 <= m <= 32.  NT: batch tiles of 8 rows (1, 2 or 4).
 // Fragment layouts (PTX ISA, mma.m16n8k16, g = lane / 4, t = lane % 4): A regs = (row g | g+8) x (k 2t,2t+1 | +8);
 // B regs = (k 2t,2t+1 | +8) x (column g); D regs = (row g | g+8) x (columns 2t, 2t+1).  Here "row" is the output
 // column n of the GEMV (W tile) and "column" is the batch row.
@@ -470,7 +472,7 @@ static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CU
                                int64_t ldy, int m, int n, int k, int nslots, int blocks, int ksplit, cudaStream_t s)
 {
     if (*attr_gen != device_generation()) {       // per-device function attribute: redo after tri_init() moved to another device
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(GV_MAX_SLOTS, 16));
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(9, 32));   // the largest configuration (>= GV_MAX_SLOTS slots of 16 rows)
         if (e != cudaSuccess) return e;
         *attr_gen = device_generation();
     }
@@ -496,19 +498,20 @@ template <bool KN>
 static cudaError_t launch_gemv_rows(int m, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
                                     int nslots, int blocks, int ksplit, cudaStream_t s)
 {
-    static int gen[5] = {-1, -1, -1, -1, -1};
+    static int gen[6] = {-1, -1, -1, -1, -1, -1};
     if (m <= 1) return launch_gemv(gemv_kernel<1, KN>, &gen[0], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
     if (m <= 2) return launch_gemv(gemv_kernel<2, KN>, &gen[1], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
     if (m <= 4) return launch_gemv(gemv_kernel<4, KN>, &gen[2], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
     if (m <= 8) return launch_gemv(gemv_mma_kernel<1, KN>, &gen[3], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
-    return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    if (m <= 16) return launch_gemv(gemv_mma_kernel<2, KN>, &gen[4], 16, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
+    return launch_gemv(gemv_mma_kernel<4, KN>, &gen[5], 32, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
 }
 
 int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
                      uint16_t *y, int64_t ldy, void *stream)
 {
     if (!x || !w || !y) return fail(TRI_ERR_INVALID_ARG, "x/w/y is NULL");
-    if (m < 1 || m > 16) return fail(TRI_ERR_INVALID_ARG, "m = %d outside [1, 16]", m);
+    if (m < 1 || m > GV_MAX_ROWS) return fail(TRI_ERR_INVALID_ARG, "m = %d outside [1, %d]", m, GV_MAX_ROWS);
     if (n < 1 || k < 1) return fail(TRI_ERR_INVALID_ARG, "n = %d, k = %d must be positive", n, k);
     if (w_layout != TRI_W_NK && w_layout != TRI_W_KN) return fail(TRI_ERR_INVALID_ARG, "w_layout = %d", w_layout);
     if (k % 8 != 0) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d must be a multiple of 8", k);
@@ -537,7 +540,7 @@ int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_
     if (kn) st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, GV_COLS, GV_STAGE_K, CU_TENSOR_MAP_SWIZZLE_128B);
     else st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GV_STAGE_K, GV_COLS, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
-    const int xrows = m <= 8 ? 8 : 16;
+    const int xrows = m <= 8 ? 8 : m <= 16 ? 16 : 32;
     st = cached_tmap_2d_bf16(&xmap, x, (uint64_t)k, (uint64_t)m, (uint64_t)ldx * 2, GV_STAGE_K, xrows,
                              m <= 4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
@@ -546,10 +549,11 @@ int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_
     // the config-3 shape with the FHFMA path: 8 -> 10 slots takes m = 1 from 21.6 to 20.1 us, m = 4 from 22.9 to 21.2.  Ten
     // slots also fill the SM with two CTAs, so that no CTA of the NEXT call (programmatic dependent launch) moves in early
     // and spins on its barriers in the issue slots of the running ones.  The FHFMA path's partial-sum sets reuse the ring.
-    const int nslots = GV_MAX_SLOTS;
+    const int nslots = m <= 16 ? GV_MAX_SLOTS : 9;         // 32 rows of X per slot: nine slots of 12 KiB keep two CTAs on an SM
     static_assert((size_t)GV_MAX_SLOTS * gemv_slot_bytes(8) >= GV_PART_OFFSET + 4096 && GV_PART_OFFSET >= (size_t)16 * GV_RED_STRIDE * 4,
                   "the partial sums must fit the ring");
-    static_assert(2 * gemv_smem_bytes(GV_MAX_SLOTS, 16) <= 227 * 1024, "two CTAs per SM");
+    static_assert(gemv_smem_bytes(9, 32) >= gemv_smem_bytes(GV_MAX_SLOTS, 16) && 2 * (gemv_smem_bytes(9, 32) + 1024) <= 228 * 1024, "two CTAs per SM");
+    static_assert((size_t)9 * gemv_slot_bytes(32) >= GV_PART_OFFSET + 4 * 2048, "the partial sums of four batch tiles must fit the ring");
 
     // Fewer column blocks than two per SM: clusters of 2 or 4 along K, as long as a rank keeps at least 24 stages (a CTA's
     // fixed cost is worth ~10 stages).  Measured on 8 x 3584 x 18944 (56 column blocks): 1 / 2 / 3 / 4 / 5 / 6 / 8 ranks ->
@@ -571,5 +575,6 @@ int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_
 extern "C" int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw,
                            int w_layout, uint16_t *y, int64_t ldy, void *stream)
 {
+    if (m > 16) return tri::fail(TRI_ERR_INVALID_ARG, "m = %d outside [1, 16]", m);     // the ABI's decode batch (include/triroof.h)
     return tri::gemv_impl(m, n, k, x, ldx, w, ldw, w_layout, y, ldy, stream);
 }

@@ -5,7 +5,7 @@
 // one-CTA kernel used when A has at most 128 rows; m > 128 goes to the CTA-pair kernel of prefill_gemm_2sm.cu (256 x 256
 // pair tiles), which a short A would leave three quarters empty.
 //
-// One-CTA kernel (16 < m <= 128: chunked-prefill tails, speculative / large-batch decode; m <= 16 goes to the GEMV): weight-streaming bound, so the
+// One-CTA kernel (32 < m <= 128: chunked-prefill tails, speculative / large-batch decode; m <= 32 goes to the GEMV): weight-streaming bound, so the
 // tile is 128 x 128 — 148 tiles for n = 18944, one per SM — and when there are fewer tiles than SMs every tile is cut
 // along K into `parts` ranges (gemm_common.cuh next_work / splitk_*) so that all SMs pull on HBM.  Warp roles as in the
 // pair kernel: warp 0 TMA producer (A rows x 64 and W 128 x 64 per k-block into a 6- to 12-stage ring, 128-byte swizzle), warp 1
@@ -394,11 +394,13 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
         const uintptr_t w0 = (uintptr_t)w, w1 = w0 + ((wrows - 1) * (size_t)ldw + wcols) * 2;
         if ((c0 < a1 && a0 < c1) || (c0 < w1 && w0 < c1)) return fail(TRI_ERR_INVALID_ARG, "c aliases an input");
     }
-    // At most 16 rows: the contraction is a weight stream with a sliver of arithmetic, and the streaming GEMV (two CTAs per
-    // SM, warp-level MMA, no TMEM set-up, no epilogue to speak of) does it in 21.5 us back to back on 16 x 18944 x 3584
-    // where the 128-row tcgen05 tile below needs 23.7 us.  Same definition, same rounding; every argument rule of this
-    // entry point is at least as strict as the GEMV's.
-    if (m <= 16) return gemv_impl(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream);
+    // At most 32 rows: the contraction is a weight stream with a sliver of arithmetic, and the streaming GEMV (two CTAs per
+    // SM, warp-level MMA with the batch as 8-column tiles, no TMEM set-up, no epilogue to speak of, K-split clusters when
+    // there are few columns) does it faster than the 128-row tcgen05 tile below.  Back to back, us, GEMV / one-CTA kernel:
+    // 16 x 18944 x 3584 21.5 / 23.7, 32 x 18944 x 3584 22.5 / 23.5, 32 x 3584 x 18944 25.5 / 29.0.  Same definition, same
+    // rounding; every argument rule of this entry point is at least as strict as the GEMV's.  (Beyond 32 rows the X
+    // fragments cost more shared-memory bandwidth than the SM has: 2 x ldmatrix.x4 per batch tile and stage in every warp.)
+    if (m <= 32) return gemv_impl(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream);
 
     const DeviceInfo *di = nullptr;
     int st = ensure_init(&di);

@@ -176,10 +176,10 @@ def test_down_projection_sampled_rows(layout):
 
 
 @pytest.mark.parametrize("layout", LAYOUTS)
-@pytest.mark.parametrize("m", [16, 24, 64, 128])
+@pytest.mark.parametrize("m", [16, 24, 32, 40, 64, 128])
 def test_short_a_up_projection(layout, m):
-    """16 < m <= 128 runs the one-CTA kernel (128 x 128 tiles; m = 24: a 24-row A box), m <= 16 is handed to the streaming
-    GEMV: the config-4 weights with a short A; 148 tiles, no split."""
+    """32 < m <= 128 runs the one-CTA kernel (128 x 128 tiles; m = 40: a 40-row A box), m <= 32 is handed to the streaming
+    GEMV (m = 24, 32: four batch tiles): the config-4 weights with a short A; 148 tiles, no split."""
     k, n = 3584, 18944
     a = normal_bf16(3, (m, k), 1.0, stream=4)
     w = normal_bf16(3, (k, n), 0.02, stream=1)
@@ -193,7 +193,9 @@ def test_short_a_up_projection(layout, m):
 @pytest.mark.parametrize("layout", LAYOUTS)
 @pytest.mark.parametrize("m,n,k", [(64, 3584, 18944),     # down-projection, 28 tiles cut 5 ways (59-60 k-blocks each)
                                    (100, 304, 1024),      # 3 tiles cut 16 ways, one k-block each
-                                   (17, 136, 4104),       # ragged last k-block, 2 tiles cut 65 ways
+                                   (40, 136, 4104),       # ragged last k-block, 2 tiles cut 65 ways
+                                   (17, 136, 4104),       # m <= 32: the GEMV's K-split clusters, four batch tiles, ragged last stage
+                                   (32, 3584, 18944),     # down-projection at 32 rows: GEMV, clusters of 4 along K
                                    (128, 19000, 640)])    # 149 tiles: one round + 1 tile cut 10 ways
 def test_one_cta_kernel_split_k(layout, m, n, k):
     a = normal_bf16(92, (m, k))
