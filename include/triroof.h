@@ -125,9 +125,9 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
  * Outputs must not alias inputs.  Asynchronous: one kernel on `stream` (two when the shape is split along k: the
  * second adds the fp32 partial tiles in a fixed order).
  * m <= 32 is computed by decode_gemv's streaming kernels (same definition and rounding).
- * For m <= 128 the kernel is launched with programmatic stream serialization, like decode_gemv: it prefetches W
- * (model state) while the kernel before it on `stream` drains, and reads A / writes C only after that kernel has
- * completed.  W must therefore not be an output of the immediately preceding prefill_gemm / decode_gemv call on
+ * The kernels are launched with programmatic stream serialization, like decode_gemv: a call sets itself up while the
+ * kernel before it on `stream` drains and, for m <= 128, prefetches W (model state) meanwhile; it reads A / writes C
+ * only after that kernel has completed.  W must therefore not be an output of the immediately preceding prefill_gemm / decode_gemv call on
  * the same stream (any other producer of W is ordered as usual).
  */
 int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,

@@ -64,7 +64,9 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
     const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
     const int ntiles = p.tiles_m * p.tiles_n;             // pair tiles (tiles_m counts 256-row blocks)
 
-    if (p.parts > 1) ptx::pdl_launch_dependents();        // splitk_reduce_kernel may take its place; it waits for this grid
+    // Programmatic dependent launch: the next kernel of the stream (splitk_reduce_kernel when this call is split, else the next
+    // call's kernel) may set itself up as SMs free up; it orders itself with griddepcontrol.wait, as this one does below.
+    ptx::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < G2_STAGES; ++s) {
             ptx::mbar_init(full0 + 8 * s, 1);             // leader's copy is the one used
@@ -98,6 +100,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
             const uint64_t pol_a = ptx::policy_evict_last();
             uint32_t it = 0;
             GemmWork wk;
+            ptx::pdl_wait();                                          // A may be the output of the grid before this one
             for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i) {
                 int tm, tn;
                 tile_coords(p, wk.tile, tm, tn);
@@ -157,6 +160,7 @@ gemm_2sm_kernel(const __grid_constant__ CUtensorMap amap, const __grid_constant_
         const uint32_t stage0 = outbuf + ew * 8192;
         uint32_t tcount = 0, sb = 0;
         if (lane == 0) ptx::prefetch_tmap(&cmap);
+        ptx::pdl_wait();                                              // C / the workspace may still be in use by the grid before
         const uint64_t pol_c = ptx::policy_evict_first();
         GemmWork wk;
         for (int i = 0; next_work(p, ntiles, pair, npairs, i, wk); ++i, ++tcount) {
@@ -277,8 +281,17 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
         if (st != TRI_OK) return st;
         if (q.full_tiles == 0) pairs = left * parts;
     }
-    gemm_2sm_kernel<<<2 * pairs, G2_THREADS, G2_SMEM_BYTES, s>>>(amap, wmap, cmap, q);
-    TRI_CUDA(cudaGetLastError());
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * pairs);
+    cfg.blockDim = dim3(G2_THREADS);
+    cfg.dynamicSmemBytes = G2_SMEM_BYTES;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_2sm_kernel, amap, wmap, cmap, q));
     if (q.parts > 1) return launch_splitk_reduce(q, 2 * G2_BM, G2_BN, true, s);
     return TRI_OK;
 }

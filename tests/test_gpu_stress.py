@@ -94,9 +94,10 @@ def test_gemv_then_gemm_then_gemv_chain():
     assert all(torch.equal(y, ys[0]) for y in ys) and all(torch.equal(c, cs[0]) for c in cs)
 
 
-@pytest.mark.parametrize("m,n", [(16, 1024), (100, 640), (128, 2048)])
+@pytest.mark.parametrize("m,n", [(16, 1024), (100, 640), (128, 2048), (300, 768), (1000, 512)])
 def test_short_gemm_chain_orders_its_data_under_pdl(m, n):
-    """prefill_gemm for m <= 128 launches with programmatic stream serialization: call i + 1 starts (and prefetches W) while
+    """prefill_gemm launches with programmatic stream serialization (GEMV kernels for m <= 32, the one-CTA kernel to 128 rows,
+    the CTA-pair kernel with its tail split and reduction kernel above): call i + 1 starts (and, for m <= 128, prefetches W) while
     call i drains, but may read A only after call i completed.  Here A of call i + 1 IS the output of call i (k = n, a
     permutation-like W keeps the values bounded): C_{i+1} = C_i . W.  The chain without any host synchronisation must equal,
     bit for bit, the same chain with a synchronisation after every call."""
