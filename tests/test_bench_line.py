@@ -117,3 +117,13 @@ def test_controller_preview_on_a_synthetic_sweep():
     d = out["eq6_decode_phase"]
     assert d["feasible"] and 1005.0 <= d["f_selected_mhz"] <= 1650.0
     json.dumps(out)
+
+
+def test_compact_line_sheds_optional_keys_rather_than_outgrow_the_tail():
+    full = mock_full()
+    full["config"]["workload"] = full["config"]["workload"] + " " + "x" * 600          # something made the line longer than planned
+    line = bench.compact_line(full)
+    d = json.loads(line)
+    assert len(line) <= 2800 and "sustained_cols" not in d
+    for k in REQUIRED:
+        assert k in d, k
