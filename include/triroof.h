@@ -104,7 +104,7 @@ int roofline_run_k(unsigned k, float a, float b, size_t n, const float *in, floa
  * k % 8 == 0.  x: device, bf16 X[i * ldx + kk], ldx >= k, ldx % 8 == 0.
  * w: device, bf16, layout w_layout (TRI_W_NK: ldw >= k; TRI_W_KN: ldw >= n), ldw % 8 == 0.
  * y: device, bf16 Y[i * ldy + j], ldy >= n.  x, w 16-byte aligned; y 2-byte aligned (any ldy).
- * Outputs must not alias inputs.  Asynchronous: one kernel per 8 rows of X on `stream`.
+ * Outputs must not alias inputs.  Asynchronous: one kernel on `stream`, whatever m is (W is read once).
  * The kernel is launched with programmatic stream serialization: it prefetches W (model state) while
  * the kernel before it on `stream` drains, and reads X / writes Y only after that kernel has completed.
  * W must therefore not be an output of the immediately preceding decode_gemv call on the same stream
@@ -127,8 +127,8 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
  * m <= 32 is computed by decode_gemv's streaming kernels (same definition and rounding).
  * The kernels are launched with programmatic stream serialization, like decode_gemv: a call sets itself up while the
  * kernel before it on `stream` drains and, for m <= 128, prefetches W (model state) meanwhile; it reads A / writes C
- * only after that kernel has completed.  W must therefore not be an output of the immediately preceding prefill_gemm / decode_gemv call on
- * the same stream (any other producer of W is ordered as usual).
+ * only after that kernel has completed.  W must therefore not be an output of the immediately preceding
+ * prefill_gemm / decode_gemv call on the same stream (any other producer of W is ordered as usual).
  */
 int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
                  int w_layout, uint16_t *c, int64_t ldc, void *stream);
