@@ -133,6 +133,37 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
 int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
                  int w_layout, uint16_t *c, int64_t ldc, void *stream);
 
+/* a3, for callers that cannot allocate.  prefill_gemm keeps the fp32 partial tiles of a shape that is split along k in
+ * a per-stream workspace which it cudaMalloc's on first use (and re-allocates when a larger shape arrives).  Some
+ * callers cannot live with that: a serving loop inside a memory pool that owns all of HBM and treats any cudaMalloc
+ * outside it as an error (or runs with so little left that one fails); code running while another stream of the process
+ * is being captured into a CUDA graph, when an allocation aborts the capture; a real-time or latency-bounded thread, for
+ * which cudaMalloc's device-wide synchronisation and unbounded duration are not acceptable; a sandboxed plug-in whose
+ * host forbids the allocator.  prefill_gemm_static_ws is the same contraction, same definition, same kernels and the same
+ * bits of C as prefill_gemm, for 33 <= m <= 128 (the one-CTA kernel: the short-A / chunked-prefill-tail case), with the
+ * partial tiles in an array that is part of the library image instead:
+ *   - the array is static device memory of 148 partial tiles x 128 x 128 fp32 = 9 699 328 bytes (9.25 MiB), 256-byte
+ *     aligned.  Every GPU on which the process loads this library holds those bytes until the process exits, whether
+ *     this entry point is ever called or not.  That is the price of the entry point and the reason the size is modest.
+ *   - the call allocates nothing and frees nothing, on the device or through a library routine that would; the caller
+ *     passes a, w, c as for prefill_gemm and owns them.
+ *   - limits: m outside [33, 128] is TRI_ERR_UNSUPPORTED_SHAPE (fewer rows never need scratch, more rows use the
+ *     CTA-pair kernel: call prefill_gemm); so is a shape whose partial tiles exceed the array, which the message
+ *     spells out in bytes (the need is at most one tile per SM, so it cannot happen on a 148-SM B200 and can on a
+ *     device with more SMs).  Every other argument rule and error is prefill_gemm's.
+ *   - first call on a device: it looks up the array's address on the current device (cudaGetSymbolAddress) and raises
+ *     the kernel's shared-memory limit there, once; later calls on that device reuse both.  Make that first call,
+ *     with the device current, before any stream capture begins.
+ *   - ONE array serves every call, stream and thread of the process on that device.  Calls on one stream are ordered
+ *     and may follow each other freely; two calls that can run on the GPU at the same time (different streams, say)
+ *     write the same bytes and give wrong results without any error: serialise them,
+ *     or use prefill_gemm, whose workspaces are per stream.  The array keeps whatever the last call left in it;
+ *     nothing needs clearing, because every partial tile is written in full before it is read.
+ * Asynchronous: one kernel on `stream`, two when the shape is split along k, launched like prefill_gemm's (the W rule
+ * above applies). */
+int prefill_gemm_static_ws(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
+                           int w_layout, uint16_t *c, int64_t ldc, void *stream);
+
 /* ------------------------------------------------------------------------------------------------
  * a4. Phase trace (Fig. 1 bottom, Fig. 4a, P:124 NVML, P:126 event-anchored phase
  *     boundaries; BASELINE.json config 5).  All buffers here are HOST memory owned by the caller.

@@ -40,7 +40,7 @@ EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "t
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
            "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_model_validate", "tri_solve_clock",
-           "tri_fit_theta", "tri_fit_power", "tri_probe_fma_issue"]
+           "tri_fit_theta", "tri_fit_power", "tri_probe_fma_issue", "prefill_gemm_static_ws"]
 
 
 class TriError(RuntimeError):
@@ -105,6 +105,7 @@ def lib():
     gemm_args = [c_int, c_int, c_int, c_void_p, c_int64, c_void_p, c_int64, c_int, c_void_p, c_int64, c_void_p]
     L.decode_gemv.argtypes = gemm_args
     L.prefill_gemm.argtypes = gemm_args
+    L.prefill_gemm_static_ws.argtypes = gemm_args
     L.phase_trace_start.argtypes = [c_int, c_uint, POINTER(tri_sample), c_size_t, POINTER(c_void_p)]
     L.phase_trace_mark.argtypes = [c_void_p, c_int]
     L.phase_trace_stop.argtypes = [c_void_p, POINTER(c_size_t)]
@@ -205,6 +206,14 @@ def decode_gemv(m, n, k, x, ldx, w, ldw, w_layout, y, ldy, stream=None) -> None:
 def prefill_gemm(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream=None) -> None:
     _check(lib().prefill_gemm(m, n, k, _ptr(a), lda, _ptr(w), ldw, w_layout, _ptr(c), ldc, _stream(stream)),
            "prefill_gemm")
+
+
+def prefill_gemm_static_ws(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream=None) -> None:
+    """prefill_gemm for 33 <= m <= 128 that allocates no device memory: the split-K partial tiles live in a 9.25 MiB
+    static device array of the library (include/triroof.h: one array per device, shared by every call; calls that
+    overlap on the GPU race; first call on a device before any stream capture)."""
+    _check(lib().prefill_gemm_static_ws(m, n, k, _ptr(a), lda, _ptr(w), ldw, w_layout, _ptr(c), ldc, _stream(stream)),
+           "prefill_gemm_static_ws")
 
 
 def tri_sm_clock_mhz(spin_us: int = 2000, stream=None) -> float:

@@ -444,7 +444,148 @@ static int gemm_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const 
     return one_sm ? launch_gemm_1sm(amap, wmap, p, di->sm_count, s) : launch_gemm_2sm(amap, wmap, p, di->sm_count, s);
 }
 
+// ---- prefill_gemm_static_ws: the one-CTA kernel with its split-K partials in a file-scope device array ----------------
+// For callers that must not allocate device memory (see include/triroof.h).  Nothing above is touched: this is a second
+// way into gemm_1sm_kernel / splitk_reduce_kernel with GemmParams::ws pointing at g_static_ws instead of at a
+// cudaMalloc'ed per-stream buffer.  The partition (which tiles are cut along K, into how many parts) is computed exactly
+// as launch_gemm_1sm computes it, so the bits of C are those of prefill_gemm.
+//
+// Size: a split shape has `left` < sm_count leftover tiles cut into parts = sm_count / left ranges, so there are at most
+// sm_count partial tiles of 128 x 128 fp32 (64 KiB) in flight: 148 of them on a B200 = 9.25 MiB.  Every device that
+// loads libtriroof.so carries the array from module load to process exit, used or not.
+constexpr int GM_STATIC_WS_TILES = 148;
+constexpr size_t GM_STATIC_WS_BYTES = (size_t)GM_STATIC_WS_TILES * GM_BM * GM_BN * sizeof(float);
+static __device__ __align__(256) float g_static_ws[(size_t)GM_STATIC_WS_TILES * GM_BM * GM_BN];
+
+// In host code the name g_static_ws is only a handle for the runtime's symbol table, not a device address; the address
+// on the CURRENT device comes from cudaGetSymbolAddress, asked once per device and remembered here.  The same set-up sets
+// the kernel's dynamic shared memory limit on that device (launch_gemm_1sm keeps its own record of that; a first call
+// through this entry point must not depend on it).
+constexpr int GM_STATIC_WS_MAX_DEVICES = 64;
+static std::mutex g_static_ws_mu;
+static float *g_static_ws_addr[GM_STATIC_WS_MAX_DEVICES] = {};
+
+static int static_ws_on_current_device(float **ws)
+{
+    int dev = -1;
+    TRI_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= GM_STATIC_WS_MAX_DEVICES)
+        return fail(TRI_ERR_CUDA, "prefill_gemm_static_ws: device ordinal %d beyond the %d this table holds", dev, GM_STATIC_WS_MAX_DEVICES);
+    std::lock_guard<std::mutex> lk(g_static_ws_mu);
+    if (!g_static_ws_addr[dev]) {
+        void *addr = nullptr;
+        TRI_CUDA(cudaGetSymbolAddress(&addr, g_static_ws));
+        if (!addr) return fail(TRI_ERR_CUDA, "cudaGetSymbolAddress gave a null address for the static split-K scratch");
+        TRI_CUDA(cudaFuncSetAttribute(gemm_1sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_MAX));
+        g_static_ws_addr[dev] = static_cast<float *>(addr);
+    }
+    *ws = g_static_ws_addr[dev];
+    return TRI_OK;
+}
+
+static int gemm_static_ws_impl(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw, int w_layout,
+                               uint16_t *c, int64_t ldc, void *stream)
+{
+    // the argument rules of prefill_gemm, checked on the host before any CUDA call
+    if (!a || !w || !c) return fail(TRI_ERR_INVALID_ARG, "a/w/c is NULL");
+    if (m < 1 || n < 1 || k < 1) return fail(TRI_ERR_INVALID_ARG, "m = %d, n = %d, k = %d must be positive", m, n, k);
+    if (w_layout != TRI_W_NK && w_layout != TRI_W_KN) return fail(TRI_ERR_INVALID_ARG, "w_layout = %d", w_layout);
+    if (k % 8 != 0) return fail(TRI_ERR_UNSUPPORTED_SHAPE, "k = %d must be a multiple of 8", k);
+    if (lda < k || ldc < n) return fail(TRI_ERR_INVALID_ARG, "lda = %lld < k or ldc = %lld < n", (long long)lda, (long long)ldc);
+    if (ldw < (w_layout == TRI_W_NK ? k : n)) return fail(TRI_ERR_INVALID_ARG, "ldw = %lld too small", (long long)ldw);
+    if (lda % 8 != 0 || ldw % 8 != 0 || ldc % 8 != 0) return fail(TRI_ERR_ALIGNMENT, "lda, ldw, ldc must be multiples of 8 elements");
+    if (!aligned(a, 16) || !aligned(w, 16) || !aligned(c, 16)) return fail(TRI_ERR_ALIGNMENT, "a, w, c must be 16-byte aligned");
+    {
+        const uintptr_t c0 = (uintptr_t)c, c1 = c0 + ((size_t)(m - 1) * ldc + n) * 2;
+        const uintptr_t a0 = (uintptr_t)a, a1 = a0 + ((size_t)(m - 1) * lda + k) * 2;
+        const size_t wrows = w_layout == TRI_W_NK ? n : k, wcols = w_layout == TRI_W_NK ? k : n;
+        const uintptr_t w0 = (uintptr_t)w, w1 = w0 + ((wrows - 1) * (size_t)ldw + wcols) * 2;
+        if ((c0 < a1 && a0 < c1) || (c0 < w1 && w0 < c1)) return fail(TRI_ERR_INVALID_ARG, "c aliases an input");
+    }
+    // the one kernel this entry point drives is the 128-row one-CTA kernel; other row counts never use scratch memory
+    // (m <= 32) or use the CTA-pair kernel's larger partial tiles (m > 128), and both are prefill_gemm's business
+    if (m <= 32 || m > GM_BM)
+        return fail(TRI_ERR_UNSUPPORTED_SHAPE, "prefill_gemm_static_ws covers 33 <= m <= %d rows (m = %d): use prefill_gemm", GM_BM, m);
+
+    const DeviceInfo *di = nullptr;
+    int st = ensure_init(&di);
+    if (st != TRI_OK) return st;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+
+    const int a_rows = ((m + 7) / 8) * 8;
+    CUtensorMap amap, wmap;
+    st = cached_tmap_2d_bf16(&amap, a, (uint64_t)k, (uint64_t)m, (uint64_t)lda * 2, GM_BK, a_rows, CU_TENSOR_MAP_SWIZZLE_128B);
+    if (st != TRI_OK) return st;
+    GemmParams p = {};
+    p.a_box_bytes = a_rows * GM_BK * 2;
+    p.m = m; p.n = n; p.k = k;
+    p.tiles_m = 1;
+    p.tiles_n = (n + GM_BN - 1) / GM_BN;
+    p.kblocks = (k + GM_BK - 1) / GM_BK;
+    p.ldc = ldc;
+    p.c = c;
+    if (w_layout == TRI_W_NK) {
+        st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)k, (uint64_t)n, (uint64_t)ldw * 2, GM_BK, GM_BN, CU_TENSOR_MAP_SWIZZLE_128B);
+        p.b_mn_major = 0;
+        p.b_lbo = 16; p.b_sbo = 1024; p.b_kstep = 32;
+    } else {
+        st = cached_tmap_2d_bf16(&wmap, w, (uint64_t)n, (uint64_t)k, (uint64_t)ldw * 2, 64, GM_BK, CU_TENSOR_MAP_SWIZZLE_128B);
+        p.b_mn_major = 1;
+        p.b_lbo = 8192; p.b_sbo = 1024; p.b_kstep = 2048;
+    }
+    if (st != TRI_OK) return st;
+
+    // ring depth and tail split: launch_gemm_1sm's rules, restated
+    const int sm_count = di->sm_count;
+    const int stage_bytes = p.a_box_bytes + GM_B_BYTES;
+    p.stages = (GM_SMEM_MAX - 1024 - GM_BAR_BYTES) / stage_bytes;
+    if (p.stages > GM_MAX_STAGES) p.stages = GM_MAX_STAGES;
+    const int ntiles = p.tiles_n;
+    const int left = ntiles % sm_count;
+    int parts = left ? sm_count / left : 1;
+    if (parts > p.kblocks) parts = p.kblocks;
+    const bool split = parts >= 2 && (parts - 1) * p.kblocks >= 8 * parts;
+    p.full_tiles = split ? ntiles - left : ntiles;
+    p.parts = split ? parts : 1;
+    if (split) {
+        const size_t need = (size_t)left * parts * GM_BM * GM_BN * sizeof(float);
+        if (need > GM_STATIC_WS_BYTES)
+            return fail(TRI_ERR_UNSUPPORTED_SHAPE,
+                        "prefill_gemm_static_ws: this shape on %d SMs needs %zu bytes of split-K scratch, the static array holds %zu",
+                        sm_count, need, GM_STATIC_WS_BYTES);
+    }
+    // the address is looked up on every path (split or not) so that the first call on a device always does the set-up
+    float *ws = nullptr;
+    st = static_ws_on_current_device(&ws);
+    if (st != TRI_OK) return st;
+    p.ws = split ? ws : nullptr;
+    const int grid = split && p.full_tiles == 0 ? left * parts : (ntiles < sm_count ? ntiles : sm_count);
+
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(GM_THREADS);
+    cfg.dynamicSmemBytes = gm_smem_bytes(p.stages, stage_bytes);
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_1sm_kernel, amap, wmap, p));
+    // Nothing in the array has to start at zero: each partial tile is written in full (all 128 rows x 128 columns, rows
+    // beyond m included) by the CTA that owns it before splitk_reduce_kernel reads it, and the reduction reads only the
+    // left * parts tiles of THIS call.  What an earlier call left behind is never read.
+    if (split) return launch_splitk_reduce(p, GM_BM, GM_BN, false, s);
+    return TRI_OK;
+}
+
 }  // namespace tri
+
+extern "C" int prefill_gemm_static_ws(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
+                                      int w_layout, uint16_t *c, int64_t ldc, void *stream)
+{
+    return tri::gemm_static_ws_impl(m, n, k, a, lda, w, ldw, w_layout, c, ldc, stream);
+}
 
 extern "C" int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
                             int w_layout, uint16_t *c, int64_t ldc, void *stream)
