@@ -174,6 +174,8 @@ typedef struct {
     uint32_t sm_mhz, mem_mhz;   /* nvmlDeviceGetClockInfo(SM / MEM) */
     uint32_t temp_c;            /* GPU temperature */
     float power_w;              /* nvmlDeviceGetPowerUsage / 1000 */
+    uint32_t read_us;           /* how long this sample's NVML queries took (t_s is taken after them): the age bound of the
+                                 * values, and where a blocked NVML call shows up in the record */
     uint64_t energy_mj;         /* nvmlDeviceGetTotalEnergyConsumption (0 if unsupported); inside a trace polled by a thread
                                  * of its own about every 100 ms and carried forward in between (the query takes 4-13 ms
                                  * on B200, more than the 10 ms sampling period) */
@@ -182,23 +184,30 @@ typedef struct {
 
 typedef struct {
     int32_t phase;              /* TRI_PHASE_* */
-    int32_t reserved;
+    int32_t expected_samples;   /* floor((t_end_s - t_begin_s) / period): what n_samples would be at the requested cadence */
     double t_begin_s, t_end_s;  /* host clock, same origin as tri_sample.t_s */
     double gpu_ms;              /* cudaEvent time between the phase's first and last kernel (0 for idle) */
     uint64_t launches;          /* kernel launches completed in the phase */
     double flop, bytes, tokens; /* algorithmic work done (tokens: m per call) */
     double energy_j, mean_power_w, j_per_flop, j_per_byte, j_per_token;
-    float sm_mhz_mean, sm_mhz_first10, sm_mhz_last10; /* clock over the phase / its first, last 10 % */
+    float sm_mhz_mean, sm_mhz_first10, sm_mhz_last10; /* clock over the phase / over the samples stamped inside the first, last
+                                 * 10 % of [t_begin_s, t_end_s] (spans of time; 0 when that span holds no sample) */
     float temp_c_max;
-    uint32_t n_samples;
-    uint32_t reserved2;
+    uint32_t n_samples;         /* samples stamped inside [t_begin_s, t_end_s] */
+    uint32_t max_gap_us;        /* longest stretch of the phase without a sample, its two edges included */
 } tri_phase_summary;
 
 enum { TRI_PHASE_IDLE = 0, TRI_PHASE_PREFILL = 1, TRI_PHASE_DECODE = 2, TRI_PHASE_ROOFLINE = 3 };
 
 /* Low-level sampler: a host thread polls NVML every period_us (>= 1000) into buf[0..cap), tagging
  * each sample with the current phase.  *handle receives an opaque pointer.  When cap is reached
- * sampling stops silently and phase_trace_stop returns TRI_ERR_BUFFER_TOO_SMALL (data kept). */
+ * sampling stops silently and phase_trace_stop returns TRI_ERR_BUFFER_TOO_SMALL (data kept).
+ * Cadence: the period is a request, not a guarantee.  NVML queries are quick on an idle or memory-bound GPU (tens of
+ * microseconds) but were seen to take tens of milliseconds each while the prefill GEMM saturates the part, and the
+ * first query after an idle spell to block for over a second; phase_trace_start therefore issues every query once
+ * before it takes the time origin, a late sampler does not burst to catch up, and each sample records its own
+ * read_us, so that gaps are visible in the data (tri_phase_summary.max_gap_us, expected_samples) instead of assumed
+ * away. */
 int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t cap, void **handle);
 int phase_trace_mark(void *handle, int phase); /* atomic tag switch; any thread */
 int phase_trace_stop(void *handle, size_t *n_samples); /* joins the sampler thread, frees the handle */

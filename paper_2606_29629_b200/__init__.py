@@ -57,16 +57,16 @@ class tri_model(Structure):
 
 class tri_sample(Structure):
     _fields_ = [("t_s", c_double), ("phase", c_int32), ("sm_mhz", c_uint32), ("mem_mhz", c_uint32),
-                ("temp_c", c_uint32), ("power_w", c_float), ("energy_mj", c_uint64), ("clk_event_reasons", c_uint64)]
+                ("temp_c", c_uint32), ("power_w", c_float), ("read_us", c_uint32), ("energy_mj", c_uint64), ("clk_event_reasons", c_uint64)]
 
 
 class tri_phase_summary(Structure):
-    _fields_ = [("phase", c_int32), ("reserved", c_int32), ("t_begin_s", c_double), ("t_end_s", c_double),
+    _fields_ = [("phase", c_int32), ("expected_samples", c_int32), ("t_begin_s", c_double), ("t_end_s", c_double),
                 ("gpu_ms", c_double), ("launches", c_uint64), ("flop", c_double), ("bytes", c_double),
                 ("tokens", c_double), ("energy_j", c_double), ("mean_power_w", c_double), ("j_per_flop", c_double),
                 ("j_per_byte", c_double), ("j_per_token", c_double), ("sm_mhz_mean", c_float),
                 ("sm_mhz_first10", c_float), ("sm_mhz_last10", c_float), ("temp_c_max", c_float),
-                ("n_samples", c_uint32), ("reserved2", c_uint32)]
+                ("n_samples", c_uint32), ("max_gap_us", c_uint32)]
 
 
 class tri_trace_workload(Structure):
@@ -224,7 +224,7 @@ def tri_sm_clock_mhz(spin_us: int = 2000, stream=None) -> float:
 
 def _sample_dict(s: tri_sample) -> dict:
     return {"t_s": s.t_s, "phase": s.phase, "sm_mhz": s.sm_mhz, "mem_mhz": s.mem_mhz, "temp_c": s.temp_c,
-            "power_w": s.power_w, "energy_mj": s.energy_mj, "clk_event_reasons": s.clk_event_reasons}
+            "power_w": s.power_w, "read_us": s.read_us, "energy_mj": s.energy_mj, "clk_event_reasons": s.clk_event_reasons}
 
 
 def tri_nvml_sample(device: int = 0) -> dict:

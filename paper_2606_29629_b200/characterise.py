@@ -75,10 +75,26 @@ def run_trace(args):
                      "j_per_token": mean("j_per_token") if name != "idle" else None,
                      "tflops": (sum(x["flop"] for x in ss) / sum(x["gpu_ms"] for x in ss) / 1e9) if name != "idle" else None,
                      "gbs": (sum(x["bytes"] for x in ss) / sum(x["gpu_ms"] for x in ss) / 1e6) if name != "idle" else None}
+    # cadence of the sampler, from the record itself: per phase kind the samples against the nominal count, the longest gap,
+    # and the distribution of how long one sample's NVML queries took (tri_sample.read_us)
+    def pct(v, q):
+        return v[min(len(v) - 1, int(q * len(v)))] if v else None
+    cadence = {"first_sample_t_s": samples[0]["t_s"] if samples else None}
+    for name, ss in kinds.items():
+        code = ss[0]["phase"]
+        rd = sorted(x["read_us"] for x in samples if x["phase"] == code)
+        cadence[name] = {"n_samples": sum(x["n_samples"] for x in ss), "expected_samples": sum(x["expected_samples"] for x in ss),
+                         "max_gap_ms": max(x["max_gap_us"] for x in ss) / 1e3,
+                         "read_us_p50": pct(rd, 0.50), "read_us_p95": pct(rd, 0.95), "read_us_p99": pct(rd, 0.99), "read_us_max": rd[-1] if rd else None}
     doc = {"experiment": "config 5 phase trace", "seconds": args.seconds, "period_ms": 10, "n_samples": len(samples),
-           "aggregate": agg, "phases": summ,
-           "samples": [[round(s["t_s"], 3), s["phase"], s["sm_mhz"], s["temp_c"], round(s["power_w"], 1)] for s in samples],
-           "samples_columns": ["t_s", "phase", "sm_mhz", "temp_c", "power_w"]}
+           "aggregate": agg, "cadence": cadence, "phases": summ,
+           "samples": [[round(s["t_s"], 3), s["phase"], s["sm_mhz"], s["temp_c"], round(s["power_w"], 1), s["read_us"]] for s in samples],
+           "samples_columns": ["t_s", "phase", "sm_mhz", "temp_c", "power_w", "read_us"]}
+    sys.stderr.write(f"first sample at {cadence['first_sample_t_s'] * 1e3:.2f} ms\n")
+    for name in kinds:
+        c = cadence[name]
+        sys.stderr.write(f"{name:8s} samples {c['n_samples']} of {c['expected_samples']} nominal, longest gap {c['max_gap_ms']:.1f} ms, "
+                         f"NVML read p50 / p95 / p99 / max {c['read_us_p50']} / {c['read_us_p95']} / {c['read_us_p99']} / {c['read_us_max']} us\n")
     for name, a in agg.items():
         sys.stderr.write(f"{name:8s} x{a['instances']:2d}  clock mean {a['sm_mhz_mean'] or 0:6.0f} MHz (first 10 % {a['sm_mhz_first10'] or 0:6.0f}, "
                          f"last 10 % {a['sm_mhz_last10'] or 0:6.0f})  Tmax {a['temp_c_max']:.0f} C  P {a['mean_power_w'] or 0:5.0f} W"

@@ -1,5 +1,7 @@
 // Run-time NVML binding, clock-lock helpers and single-sample read (include/triroof.h: a4 helpers).
 #include "nvml_dyn.h"
+
+#include <time.h>
 #include "tri_internal.h"
 
 #include <dlfcn.h>
@@ -151,7 +153,13 @@ int tri_nvml_sample(int device, tri_sample *out)
     if (!h) return TRI_ERR_NVML_UNAVAILABLE;
     memset(out, 0, sizeof(*out));
     out->phase = -1;
-    return tri::nvml::read_sample(a, h, out);
+    timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    int st = tri::nvml::read_sample(a, h, out);
+    clock_gettime(CLOCK_MONOTONIC, &t1);
+    const double us = 1e6 * (double)(t1.tv_sec - t0.tv_sec) + 1e-3 * (double)(t1.tv_nsec - t0.tv_nsec);
+    out->read_us = us < 4.0e9 ? (uint32_t)us : 4000000000u;      // the energy query included here (4-13 ms on B200)
+    return st;
 }
 
 int tri_lock_clocks(int device, unsigned sm_mhz, unsigned mem_mhz)

@@ -11,6 +11,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <thread>
 #include <vector>
@@ -45,7 +46,16 @@ struct Tracer {
     unsigned period_us = 10000;
     double t0 = 0.0;
     std::atomic<uint64_t> energy_mj{0};
+    std::mutex energy_mu;                 // one energy query at a time: the poller below and the driver's phase-edge reads
     std::thread th, eth;
+
+    uint64_t read_energy(uint64_t fallback)
+    {
+        unsigned long long e = 0;
+        std::lock_guard<std::mutex> lk(energy_mu);
+        if (api->total_energy && api->total_energy(dev, &e) == nvml::SUCCESS) return e;
+        return fallback;
+    }
 
     // The energy counter is the one slow NVML query (4-13 ms on B200, more while the driver is busy launching): it is polled
     // by a thread of its own about every 100 ms and the sampler copies the last value, so that the clock / temperature /
@@ -55,8 +65,7 @@ struct Tracer {
         const double step = period_us >= 100000 ? 1e-6 * period_us : 0.1;
         double next = now_s();
         while (!stop.load(std::memory_order_acquire)) {
-            unsigned long long e = 0;
-            if (api->total_energy && api->total_energy(dev, &e) == nvml::SUCCESS) energy_mj.store(e, std::memory_order_release);
+            energy_mj.store(read_energy(energy_mj.load(std::memory_order_relaxed)), std::memory_order_release);
             next += step;
             const double t = now_s();
             if (next < t) next = t;
@@ -76,9 +85,12 @@ struct Tracer {
             }
             tri_sample s;
             memset(&s, 0, sizeof(s));
+            const double t_before = now_s();
             nvml::read_sample(api, dev, &s, false);
             s.energy_mj = energy_mj.load(std::memory_order_acquire);
-            s.t_s = now_s() - t0;                      // stamped after the reads: the values are at most this old
+            const double t_after = now_s();
+            s.t_s = t_after - t0;                      // stamped after the reads: the values are at most read_us old
+            s.read_us = (uint32_t)std::min((t_after - t_before) * 1e6, 4.0e9);   // a blocked NVML call shows in the record
             s.phase = phase.load(std::memory_order_acquire);
             buf[i] = s;
             n.store(i + 1, std::memory_order_release);
@@ -90,43 +102,40 @@ struct Tracer {
     }
 };
 
-// Reduces samples[0..ns) in [t_begin, t_end] into the clock / temperature fields of *out.
-static void reduce_window(const tri_sample *samples, size_t ns, tri_phase_summary *out)
+// Reduces samples[0..ns) in [t_begin, t_end] into the clock / temperature / cadence fields of *out.
+// First / last 10 % are spans of TIME, not of whatever samples there are: a window that lost its opening samples to a
+// slow NVML call reports 0 for sm_mhz_first10 instead of passing off its middle as its start (Fig. 4a, PAPER.md line 104,
+// is exactly that number).  max_gap_us counts the window's edges too: begin to first sample, last sample to end.
+static void reduce_window(const tri_sample *samples, size_t ns, double period_s, tri_phase_summary *out)
 {
-    std::vector<const tri_sample *> w;
-    for (size_t i = 0; i < ns; ++i)
-        if (samples[i].t_s >= out->t_begin_s && samples[i].t_s <= out->t_end_s) w.push_back(&samples[i]);
-    out->n_samples = (uint32_t)w.size();
-    if (w.empty()) return;
-    double sum = 0.0, tmax = 0.0;
-    for (auto *s : w) {
-        sum += s->sm_mhz;
-        if (s->temp_c > tmax) tmax = s->temp_c;
+    const double tb = out->t_begin_s, te = out->t_end_s, dur = te - tb;
+    out->expected_samples = period_s > 0 && dur > 0 ? (int32_t)std::min(std::floor(dur / period_s), 2.0e9) : 0;
+    double sum = 0.0, tmax = 0.0, f = 0.0, l = 0.0, prev = tb, gap = 0.0;
+    uint32_t n = 0, nf = 0, nl = 0;
+    for (size_t i = 0; i < ns; ++i) {
+        const tri_sample &s = samples[i];
+        if (s.t_s < tb || s.t_s > te) continue;
+        ++n;
+        sum += s.sm_mhz;
+        if (s.temp_c > tmax) tmax = s.temp_c;
+        if (s.t_s - prev > gap) gap = s.t_s - prev;
+        prev = s.t_s;
+        if (s.t_s <= tb + 0.1 * dur) { f += s.sm_mhz; ++nf; }
+        if (s.t_s >= te - 0.1 * dur) { l += s.sm_mhz; ++nl; }
     }
-    out->sm_mhz_mean = (float)(sum / (double)w.size());
+    if (te - prev > gap) gap = te - prev;
+    out->max_gap_us = (uint32_t)std::min(gap * 1e6, 4.0e9);
+    out->n_samples = n;
+    if (n == 0) return;
+    out->sm_mhz_mean = (float)(sum / (double)n);
     out->temp_c_max = (float)tmax;
-    size_t d = w.size() / 10;
-    if (d == 0) d = 1;
-    double f = 0.0, l = 0.0;
-    for (size_t i = 0; i < d; ++i) {
-        f += w[i]->sm_mhz;
-        l += w[w.size() - 1 - i]->sm_mhz;
-    }
-    out->sm_mhz_first10 = (float)(f / (double)d);
-    out->sm_mhz_last10 = (float)(l / (double)d);
-}
-
-static uint64_t energy_now_mj(const nvml::Api *a, nvml::Device h)
-{
-    unsigned long long e = 0;
-    if (a->total_energy && a->total_energy(h, &e) == nvml::SUCCESS) return e;
-    return 0;
+    out->sm_mhz_first10 = nf ? (float)(f / (double)nf) : 0.f;
+    out->sm_mhz_last10 = nl ? (float)(l / (double)nl) : 0.f;
 }
 
 }  // namespace tri
 
 extern "C" {
-
 int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t cap, void **handle)
 {
     if (!buf || !handle || cap == 0) return tri::fail(TRI_ERR_INVALID_ARG, "buf/handle is NULL or cap is 0");
@@ -142,12 +151,17 @@ int phase_trace_start(int device, unsigned period_us, tri_sample *buf, size_t ca
     t->buf = buf;
     t->cap = cap;
     t->period_us = period_us;
-    t->t0 = tri::now_s();
     tri::nvml::tracer_enter();                    // tri_shutdown() keeps NVML loaded while this sampler runs
     {
-        unsigned long long e = 0;                 // the first sample already carries a counter value
-        if (a->total_energy && a->total_energy(h, &e) == tri::nvml::SUCCESS) t->energy_mj.store(e);
+        // Every query once, BEFORE the time origin: the first NVML call after an idle spell can block for a long time (1.25 s
+        // seen on a fresh B200 lease after 1 s of idle), and that cost belongs to set-up, not to the trace.  The energy
+        // value read here is what the first samples carry.
+        tri_sample warm;
+        memset(&warm, 0, sizeof(warm));
+        tri::nvml::read_sample(a, h, &warm, false);
+        t->energy_mj.store(t->read_energy(0));
     }
+    t->t0 = tri::now_s();
     t->th = std::thread([t] { t->run(); });
     t->eth = std::thread([t] { t->run_energy(); });
     *handle = t;
@@ -224,6 +238,9 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
     }
     Tracer *tr = static_cast<Tracer *>(handle);
     const double t0 = tr->t0;
+    // The first phase begins once the sampler has delivered a sample (normally a fraction of a period; bounded at 2 s), so
+    // that the opening of the first window - the Fig. 4a number - is never lost to a slow first read.
+    for (const double tw = now_s(); tr->n.load(std::memory_order_acquire) == 0 && now_s() - tw < 2.0;) sleep_until(now_s() + 0.001);
 
     const int lda = wl->pk, ldc = wl->pn, ldx = wl->dk, ldy = wl->dn;
     const int p_ldw = wl->w_layout == TRI_W_NK ? wl->pk : wl->pn;
@@ -250,18 +267,19 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
             memset(&sm, 0, sizeof(sm));
             sm.phase = ph;
             phase_trace_mark(handle, ph);
-            const uint64_t en0 = energy_now_mj(a, h);
+            const uint64_t en0 = tr->read_energy(0);
             const double tb = now_s();
             sm.t_begin_s = tb - t0;
             if (ph == TRI_PHASE_IDLE) {
                 sleep_until(tb + dur);                  // no kernels queued, context alive, host thread blocked
             } else {
                 const unsigned depth = ph == TRI_PHASE_PREFILL ? 4u : 64u;   // launches per queue-bounding event
-                cudaEventRecord(e0, s);
+                cudaError_t ce = cudaEventRecord(e0, s);
+                if (ce != cudaSuccess) status = fail(TRI_ERR_CUDA, "cudaEventRecord: %s", cudaGetErrorString(ce));
                 uint64_t launches = 0;
                 unsigned slot = 0;
                 bool have[2] = {false, false};
-                while (now_s() - tb < dur) {
+                while (status == TRI_OK && now_s() - tb < dur) {
                     for (unsigned q = 0; q < depth; ++q) {
                         if (ph == TRI_PHASE_PREFILL)
                             status = prefill_gemm(wl->pm, wl->pn, wl->pk, wl->pa, lda, wl->pw, p_ldw, wl->w_layout, wl->pc, ldc, s);
@@ -272,14 +290,18 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
                         ++launches;
                     }
                     if (status != TRI_OK) break;
-                    cudaEventRecord(ring[slot], s);
+                    ce = cudaEventRecord(ring[slot], s);
+                    if (ce != cudaSuccess) {
+                        status = fail(TRI_ERR_CUDA, "cudaEventRecord: %s", cudaGetErrorString(ce));
+                        break;
+                    }
                     have[slot] = true;
                     slot ^= 1;
                     if (have[slot]) cudaEventSynchronize(ring[slot]);   // at most 2 * depth launches in flight
                 }
-                cudaEventRecord(e1, s);
-                cudaError_t ce = cudaEventSynchronize(e1);
-                if (ce != cudaSuccess && status == TRI_OK) status = fail(TRI_ERR_CUDA, "phase sync: %s", cudaGetErrorString(ce));
+                ce = cudaEventRecord(e1, s);
+                if (ce == cudaSuccess) ce = cudaEventSynchronize(e1);
+                if (ce != cudaSuccess && status == TRI_OK) status = fail(TRI_ERR_CUDA, "phase end: %s", cudaGetErrorString(ce));
                 float ms = 0.f;
                 if (status == TRI_OK) cudaEventElapsedTime(&ms, e0, e1);
                 sm.gpu_ms = ms;
@@ -291,7 +313,7 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
                 sm.tokens = (double)(ph == TRI_PHASE_PREFILL ? wl->pm : wl->dm) * (double)launches;
             }
             const double te = now_s();
-            const uint64_t en1 = energy_now_mj(a, h);
+            const uint64_t en1 = tr->read_energy(0);
             sm.t_end_s = te - t0;
             sm.energy_j = en1 >= en0 ? 1e-3 * (double)(en1 - en0) : 0.0;
             if (nsum < scap) summaries[nsum++] = sm;
@@ -304,7 +326,7 @@ int phase_trace(const tri_trace_workload *wl, double total_s, double prefill_s, 
     *n_samples = ns;
     for (size_t i = 0; i < nsum; ++i) {
         tri_phase_summary *q = &summaries[i];
-        reduce_window(samples, ns, q);
+        reduce_window(samples, ns, 1e-3 * period_ms, q);
         const double dt = q->t_end_s - q->t_begin_s;
         if (q->energy_j <= 0.0 && q->n_samples > 0) {          // no energy counter: integrate the power samples
             double pw = 0.0;
