@@ -25,7 +25,11 @@
  *   - CUDA graphs: the compute calls (roofline_run, decode_gemv, prefill_gemm) enqueue kernels only, so a sequence of
  *     them can be captured in a CUDA graph once each distinct call has run once on the capture stream (a prefill_gemm
  *     shape that is split along k allocates that stream's fp32 workspace on first use, which capture does not allow);
- *     replays give the bits of the eager calls (tested).
+ *     replays give the bits of the eager calls (tested).  A graph captured from a split shape holds the ADDRESS of
+ *     that stream's workspace in its kernel parameters: it must not be replayed after tri_shutdown() (which frees the
+ *     workspaces, also when it leaves NVML loaded because a trace is running) nor after a later, larger split shape on
+ *     the same stream has made the workspace grow (free + allocate; shapes up to 20 MB of partials - every shape with
+ *     n, m as in configs 3-4 - never grow it).  Re-capture after either.
  *   - There is no CPU fallback: a device that is not compute capability 10.x yields TRI_ERR_ARCH.
  *   - bf16 values are passed as raw uint16_t bit patterns.
  */
@@ -107,8 +111,13 @@ int roofline_run_k(unsigned k, float a, float b, size_t n, const float *in, floa
  * Outputs must not alias inputs.  Asynchronous: one kernel on `stream`, whatever m is (W is read once).
  * The kernel is launched with programmatic stream serialization: it prefetches W (model state) while
  * the kernel before it on `stream` drains, and reads X / writes Y only after that kernel has completed.
- * W must therefore not be an output of the immediately preceding decode_gemv call on the same stream
- * (any other producer of W is ordered as usual).
+ * W must therefore not be written by the kernel that immediately precedes the call on `stream`, whatever its origin
+ * (a decode_gemv / prefill_gemm of this library, or a caller's dequantisation, weight update or cache append): under
+ * programmatic serialization a predecessor's writes are guaranteed visible only after griddepcontrol.wait, and W is
+ * fetched before it.  Any earlier producer of W is ordered as usual.  A caller that does produce W right before the
+ * call puts any other kernel in between, or runs the process with the environment variable TRI_PDL=0 (read once, at the
+ * first launch): every kernel of the library is then launched without the attribute and starts only after its
+ * predecessor has completed (tested; costs the overlap, about 1-2 us per call).
  */
 int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw,
                 int w_layout, uint16_t *y, int64_t ldy, void *stream);
@@ -127,8 +136,9 @@ int decode_gemv(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint1
  * m <= 32 is computed by decode_gemv's streaming kernels (same definition and rounding).
  * The kernels are launched with programmatic stream serialization, like decode_gemv: a call sets itself up while the
  * kernel before it on `stream` drains and, for m <= 128, prefetches W (model state) meanwhile; it reads A / writes C
- * only after that kernel has completed.  W must therefore not be an output of the immediately preceding
- * prefill_gemm / decode_gemv call on the same stream (any other producer of W is ordered as usual).
+ * only after that kernel has completed.  The rule on W stated for decode_gemv holds here for every m (m <= 32 runs
+ * decode_gemv's kernels): W must not be written by the kernel immediately preceding the call on `stream`; TRI_PDL=0
+ * lifts it.
  */
 int prefill_gemm(int m, int n, int k, const uint16_t *a, int64_t lda, const uint16_t *w, int64_t ldw,
                  int w_layout, uint16_t *c, int64_t ldc, void *stream);
@@ -247,13 +257,6 @@ int tri_nvml_sample(int device, tri_sample *out);
 /* SM clock seen from inside the GPU: a one-block kernel spins for about spin_us microseconds and
  * returns delta(clock64) / delta(globaltimer ns) * 1000 in *mhz.  Blocking (synchronises stream). */
 int tri_sm_clock_mhz(unsigned spin_us, double *mhz, void *stream);
-
-/* Machine probe: issue cost of the mixed-precision FMA (fma.rn.f32.bf16, SASS FHFMA.BF16) by operand
- * pattern.  pattern 0: both bf16 operands repeat between consecutive FMAs (only the accumulator register is fetched);
- * 1: one repeats and the two fetched registers have the same parity; 2: operands repeat only every other instruction.
- * sm_mhz: the SM clock to convert time into cycles (read it with tri_sm_clock_mhz or NVML).  *cycles_per_fma: issue
- * cycles per warp-level FMA on one SM sub-partition.  Blocking; allocates and frees 12 KiB of device memory. */
-int tri_probe_fma_issue(int pattern, double sm_mhz, double *cycles_per_fma, void *stream);
 
 /* ------------------------------------------------------------------------------------------------
  * f3. A.I.-aware frequency selection (section III-C): the throughput and power

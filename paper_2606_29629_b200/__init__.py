@@ -40,7 +40,7 @@ EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "t
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
            "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_model_validate", "tri_solve_clock",
-           "tri_fit_theta", "tri_fit_power", "tri_probe_fma_issue", "prefill_gemm_static_ws"]
+           "tri_fit_theta", "tri_fit_power", "prefill_gemm_static_ws"]
 
 
 class TriError(RuntimeError):
@@ -118,7 +118,6 @@ def lib():
     L.tri_sm_clock_mhz.argtypes = [c_uint, POINTER(c_double), c_void_p]
     L.tri_fit_power.argtypes = [POINTER(c_double), POINTER(c_double), POINTER(c_double), c_size_t, POINTER(tri_model), c_double, c_double,
                                 c_double, POINTER(c_double), POINTER(c_double), POINTER(c_size_t)]
-    L.tri_probe_fma_issue.argtypes = [c_int, c_double, POINTER(c_double), c_void_p]
     for name in ("tri_model_theta", "tri_model_phi"):
         getattr(L, name).argtypes = [POINTER(tri_model), c_double, c_double]
         getattr(L, name).restype = c_double
@@ -304,6 +303,7 @@ class Model:
 
     def __init__(self, eta, beta, omega=0.0, gamma=0.0, p_tdp=1000.0, f_mhz=(), p_idle_w=(), p_dyn_w=()):
         n = len(f_mhz)
+        self._validated = set()
         self._f = (c_double * n)(*f_mhz)
         self._pi = (c_double * n)(*p_idle_w)
         self._pd = (c_double * n)(*p_dyn_w)
@@ -323,8 +323,13 @@ class Model:
         """The premise of solve_clock at this A.I. (tables well formed, theta and power monotone in f); raises TriError."""
         _check(lib().tri_model_validate(byref(self.c), ai), "tri_model_validate")
 
-    def solve_clock(self, ai, f_limit_mhz, eps):
-        """Eq. 6 -> (index into f_mhz, feasible)."""
+    def solve_clock(self, ai, f_limit_mhz, eps, check=True):
+        """Eq. 6 -> (index into f_mhz, feasible).  check=True runs tri_model_validate the first time this Model sees this
+        A.I. (O(n_f), remembered: the tables of a Model do not change) and raises TriError on tables the binary search is
+        not exact on; check=False is the bare O(log n_f) C call for callers that validated themselves."""
+        if check and ai not in self._validated:
+            self.validate(ai)
+            self._validated.add(ai)
         idx, feas = c_int32(-1), c_int32(0)
         _check(lib().tri_solve_clock(byref(self.c), ai, f_limit_mhz, eps, byref(idx), byref(feas)), "tri_solve_clock")
         return idx.value, bool(feas.value)
@@ -342,13 +347,6 @@ def tri_fit_theta(ai, f_mhz, theta, ai_mem, ai_cmp, gamma=0.0):
     _check(lib().tri_fit_theta((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*theta), n, ai_mem, ai_cmp, gamma,
                                byref(m)), "tri_fit_theta")
     return {"eta": m.eta, "beta": m.beta, "omega": m.omega, "gamma": m.gamma}
-
-
-def tri_probe_fma_issue(pattern: int, sm_mhz: float, stream=None) -> float:
-    """Issue cycles per FHFMA.BF16 for operand pattern 0 / 1 / 2 (include/triroof.h)."""
-    v = c_double(0.0)
-    _check(lib().tri_probe_fma_issue(pattern, sm_mhz, byref(v), _stream(stream)), "tri_probe_fma_issue")
-    return v.value
 
 
 def tri_fit_power(ai, f_mhz, p_w, eta, beta, f_sel_mhz, f_tol_mhz, p_cap_w):
@@ -378,8 +376,8 @@ def tri_model_validate(model: Model, ai: float) -> None:
     model.validate(ai)
 
 
-def tri_solve_clock(model: Model, ai: float, f_limit_mhz: float, eps: float):
-    return model.solve_clock(ai, f_limit_mhz, eps)
+def tri_solve_clock(model: Model, ai: float, f_limit_mhz: float, eps: float, check: bool = True):
+    return model.solve_clock(ai, f_limit_mhz, eps, check)
 
 
 # the remaining C names, as thin aliases of the wrappers above

@@ -13,7 +13,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["core.cu", "fma_chain.cu", "decode_gemv.cu", "prefill_gemm.cu", "prefill_gemm_2sm.cu", "nvml_dyn.cu", "phase_trace.cu", "dvfs_model.cu", "probe_regbank.cu"]
+SOURCES = ["core.cu", "fma_chain.cu", "decode_gemv.cu", "prefill_gemm.cu", "prefill_gemm_2sm.cu", "nvml_dyn.cu", "phase_trace.cu", "dvfs_model.cu"]
 HEADERS = ["tri_internal.h", "ptx.cuh", "gemm_common.cuh", "nvml_dyn.h", os.path.join("..", "..", "include", "triroof.h")]
 LIB = os.path.join(HERE, "libtriroof.so")
 OBJDIR = os.path.join(HERE, "build")

@@ -3,6 +3,7 @@
 #include "tri_internal.h"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -56,6 +57,15 @@ static int init_locked(int device)
 }
 
 int device_generation() { return g_generation; }
+
+int pdl_allowed()
+{
+    static const int v = [] {
+        const char *e = getenv("TRI_PDL");
+        return (e && e[0] == '0' && e[1] == 0) ? 0 : 1;
+    }();
+    return v;
+}
 
 int ensure_init(const DeviceInfo **info)
 {

@@ -1,5 +1,5 @@
 // a2. Decode-phase GEMV ("GEMV-like operators"; BASELINE.json config 3; ABI in
-// include/triroof.h):   Y[m][n] = bf16_rne( sum_k X[m][k] * W[k][n] ),  m <= 16, fp32 accumulation.
+// include/triroof.h):   Y[m][n] = bf16_rne( sum_k X[m][k] * W[k][n] ),  m <= 32 here (decode_gemv's ABI: m <= 16), fp32 accumulation.
 //
 // HBM-bound: the weight matrix is read exactly once, whatever m is.  One skeleton, both layouts: a CTA owns 64 output
 // columns; 4 compute warps + 1 producer warp (160 threads), TWO CTAs per SM (18944 = 296 * 64: one wave on 148 SMs),
@@ -483,7 +483,7 @@ static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CU
     cfg.stream = s;
     cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl_allowed();
     attr[1].id = cudaLaunchAttributeClusterDimension;
     attr[1].val.clusterDim.x = ksplit;
     attr[1].val.clusterDim.y = 1;

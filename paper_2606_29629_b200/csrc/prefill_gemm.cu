@@ -275,7 +275,7 @@ int launch_splitk_reduce(const GemmParams &p, int tile_rows, int tile_cols, bool
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl_allowed();
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     TRI_CUDA(cudaLaunchKernelEx(&cfg, splitk_reduce_kernel, p, tile_rows, tile_cols, pair_order ? 1 : 0));
@@ -368,7 +368,7 @@ static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, con
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl_allowed();
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_1sm_kernel, amap, wmap, q));
@@ -568,7 +568,7 @@ static int gemm_static_ws_impl(int m, int n, int k, const uint16_t *a, int64_t l
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl_allowed();
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_1sm_kernel, amap, wmap, p));

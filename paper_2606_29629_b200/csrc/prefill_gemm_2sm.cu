@@ -288,7 +288,7 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
     cfg.stream = s;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl_allowed();
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     TRI_CUDA(cudaLaunchKernelEx(&cfg, gemm_2sm_kernel, amap, wmap, cmap, q));

@@ -36,9 +36,15 @@ int make_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64
 int cached_tmap_2d_bf16(CUtensorMap *map, const void *base, uint64_t inner, uint64_t outer,
                         uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_outer, CUtensorMapSwizzle swz);
 
-// decode_gemv.cu: the streaming GEMV (1 <= m <= 16) behind decode_gemv(); prefill_gemm() hands it an A of at most 16 rows.
+// decode_gemv.cu: the streaming GEMV (1 <= m <= 32 = GV_MAX_ROWS) behind decode_gemv(), whose ABI stops at 16 rows;
+// prefill_gemm() hands it an A of at most 32 rows.
 int gemv_impl(int m, int n, int k, const uint16_t *x, int64_t ldx, const uint16_t *w, int64_t ldw, int w_layout,
               uint16_t *y, int64_t ldy, void *stream);
+
+// Launch attribute value for programmatic stream serialization: 1, or 0 when the environment has TRI_PDL=0 (read once).
+// With 0 every kernel of the library starts only after the kernel before it on the stream has completed and flushed,
+// so W may be produced by that kernel (include/triroof.h, decode_gemv); the griddepcontrol instructions become no-ops.
+int pdl_allowed();
 
 inline bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 

@@ -63,7 +63,9 @@ def test_solver_binary_search_equals_exhaustive_search():
             assert any(b < a for a, b in zip(th, th[1:])) or any(b < a for a, b in zip(pw, pw[1:]))
             rejected += 1
             top = max(i for i, x in enumerate(f) if x <= f_limit)
-            idx, _ = m.solve_clock(ai, f_limit, eps)    # unvalidated tables: still a legal index, not necessarily the optimum
+            with pytest.raises(tri.TriError):           # the wrapper validates on first use of an A.I. and refuses too
+                m.solve_clock(ai, f_limit, eps)
+            idx, _ = m.solve_clock(ai, f_limit, eps, check=False)    # bare C call on unvalidated tables: still a legal index, not necessarily the optimum
             assert 0 <= idx <= top
             continue
         got = m.solve_clock(ai, f_limit, eps)

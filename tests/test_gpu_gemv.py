@@ -82,8 +82,8 @@ def test_config3_shape_other_batch_sizes(layout, m):
 @pytest.mark.parametrize("m", [1, 2, 4, 5, 8, 16])
 def test_down_projection_shape_full_output(layout, m):
     """The Thinker MLP down-projection at decode batch sizes (18944 -> 3584): 56 column blocks, so the launch
-    is a grid of 5-CTA clusters along K (59-60 stages per rank through the 10-slot ring, partial sums through distributed
-    shared memory); every kernel of both paths; full output, stated bound."""
+    is a grid of 4-CTA clusters along K (gemv_impl picks 1, 2 or 4 ranks; 74 stages per rank through the 10-slot ring,
+    partial sums through distributed shared memory); every kernel of both paths; full output, stated bound."""
     k, n = 18944, 3584
     x = normal_bf16(2, (m, k), 1.0, stream=8)
     w = normal_bf16(2, (k, n), 0.02, stream=9)

@@ -196,3 +196,50 @@ def test_calls_are_capturable_in_a_cuda_graph():
         s.synchronize()
     for a, b in zip(ref, outs):
         assert torch.equal(a, b)
+
+
+_W_PRODUCER_SCRIPT = r"""
+import numpy as np, torch
+import paper_2606_29629_b200 as tri
+from synth_inputs import normal_bf16
+
+def dev(bits):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda()
+
+k, n = 3584, 4608
+srcs = [dev(np.ascontiguousarray(normal_bf16(130 + i, (k, n), 0.03).T)) for i in range(2)]     # physical [n][k]
+w = torch.zeros_like(srcs[0])
+for m, fn in ((8, tri.decode_gemv), (64, tri.prefill_gemm), (300, tri.prefill_gemm)):
+    x = dev(normal_bf16(140 + m, (m, k)))
+    want = []
+    for s in srcs:                                   # the product for each W, computed with everything synchronised
+        w.copy_(s); torch.cuda.synchronize()
+        y = torch.zeros((m, n), dtype=torch.int16, device="cuda")
+        fn(m, n, k, x, k, w, k, tri.TRI_W_NK, y, n); torch.cuda.synchronize()
+        want.append(y.clone())
+    assert not torch.equal(want[0], want[1])
+    outs = []
+    for it in range(24):                             # W rewritten by a plain kernel DIRECTLY before each call, no sync anywhere
+        y = torch.full((m, n), 0x7FC0, dtype=torch.int16, device="cuda")
+        w.copy_(srcs[it & 1])
+        fn(m, n, k, x, k, w, k, tri.TRI_W_NK, y, n)
+        outs.append(y)
+    torch.cuda.synchronize()
+    for it, y in enumerate(outs):
+        assert torch.equal(y, want[it & 1]), (m, it, int((y != want[it & 1]).sum()))
+print("ok")
+"""
+
+
+def test_w_written_by_the_preceding_kernel_with_pdl_off():
+    """include/triroof.h, decode_gemv: with the environment's TRI_PDL=0 the kernels are launched without programmatic
+    stream serialization, so a W produced by the kernel directly before the call (here a device-to-device copy kernel,
+    alternating between two weight matrices, 24 calls with no synchronisation) is the W the call reads.  The variable is
+    read once per process, hence the subprocess."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, TRI_PDL="0", PYTHONPATH=root + os.pathsep + os.environ.get("PYTHONPATH", ""))
+    r = subprocess.run([sys.executable, "-c", _W_PRODUCER_SCRIPT], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and r.stdout.strip().endswith("ok"), (r.stdout[-500:], r.stderr[-3000:])
