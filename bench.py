@@ -39,8 +39,12 @@ PAPER_KS = [4, 100, 200, 400, 800]      # the paper's own A.I. set {1, 25, 50, 1
 RIDGE_KS = [24, 40, 48, 96]             # between the powers of two around the ridge (A.I. 6 .. 24), where the sweep is weakest
 # Thinker-shaped GEMMs beside config 4: label -> (m, n, k)
 GEMM_SHAPES = {"down_proj": (4096, 3584, 18944), "qkv": (4096, 4608, 3584), "o_proj": (4096, 3584, 3584),
-               "up_m512": (512, 18944, 3584), "up_m128": (128, 18944, 3584), "up_m64": (64, 18944, 3584),
+               "up_m512": (512, 18944, 3584), "up_m256": (256, 18944, 3584), "up_m128": (128, 18944, 3584), "up_m64": (64, 18944, 3584),
                "up_m16": (16, 18944, 3584), "down_m64": (64, 3584, 18944)}
+# Decode-size GEMVs of one Thinker layer ("GEMV-like operators"): label -> (m, n, k)
+GEMV_SHAPES = {"qkv_m8": (8, 4608, 3584), "o_proj_m8": (8, 3584, 3584), "up_m8": (8, 18944, 3584), "down_m8": (8, 3584, 18944),
+               "up_m1": (1, 18944, 3584)}
+DECODE_LAYER = ["qkv_m8", "o_proj_m8", "up_m8", "down_m8"]     # the GEMVs of one layer at decode batch 8, back to back
 NOMINAL_HBM_GBS = 8000.0               # BASELINE.json north_star "roughly 8 TB/s" (context; `frac` uses the measured peaks)
 NOMINAL_BF16_TFLOPS = 2250.0           # dense bf16, nominal
 FP32_LANES_PER_SM = 128                # FP32 FMA lanes per SM (4 SMSPs x 32); DESIGN.md "ALU peak"
@@ -79,12 +83,18 @@ def load_peaks():
             "source": "fallback"}
 
 
+# The ncu --set full captures the DRAM traffic figures come from, by name (not "the newest by sort order"): re-capture
+# a kernel -> commit the new summary and change its line here.
+NCU_CAPTURES = {"fma_chain": "profiles/r2b_ncu_fma_chain.txt", "decode_gemv": "profiles/r2b_ncu_decode_gemv.txt",
+                "prefill_gemm": "profiles/r2b_ncu_prefill_gemm.txt"}
+
+
 def ncu_traffic_bytes(kernel, column):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed text summary of the ncu
-    --set full capture (profiles/<round>_ncu_<kernel>.txt, newest round); None when there is no summary."""
-    import glob
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, read from the committed text summary of that kernel's
+    ncu --set full capture (NCU_CAPTURES) - a stored figure of an earlier run of the same kernel, not measured in this
+    run (`traffic_source` on the line says which file); None when there is no summary."""
     import re
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"*_ncu_{kernel}.txt")))
+    files = [os.path.join(ROOT, NCU_CAPTURES[kernel])] if os.path.exists(os.path.join(ROOT, NCU_CAPTURES.get(kernel, "-"))) else []
     if not files:
         return None
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
@@ -270,6 +280,7 @@ def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
     except tri.TriError:
         return {}
     out, windows = {}, []
+    side = torch.cuda.Stream()
     for idx, (name, series, kk, fn, per_call, flop, nbytes) in enumerate(specs):
         est = est_ms.get(name) or (fma_flop(kk) / (0.9 * sms * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6) * 1e3 + 0.33)
         batch = max(1, int(20.0 / (est * per_call)))                  # about 20 ms of work per host round trip
@@ -280,17 +291,25 @@ def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
         t0 = time.perf_counter()
         a.record()
         calls = 0
+        clk_in_kernel = None
         while time.perf_counter() - t0 < seconds:
             for _ in range(batch):
                 fn()
             calls += batch * per_call
+            if clk_in_kernel is None and time.perf_counter() - t0 >= 0.5 * seconds:
+                # the SM clock seen from inside the GPU, per point and UNDER this point's load - the one-block
+                # clock64 / globaltimer probe runs on a side stream beside the batch just enqueued (blocks ~2 ms)
+                try:
+                    clk_in_kernel = tri.tri_sm_clock_mhz(2000, stream=side)
+                except tri.TriError:
+                    clk_in_kernel = 0.0
             torch.cuda.synchronize()
         b.record()
         torch.cuda.synchronize()
         e1 = tri.tri_nvml_sample(local)["energy_mj"]
-        windows.append((name, series, kk, 100 + idx, a.elapsed_time(b), calls, flop, nbytes, (e1 - e0) * 1e-3))
+        windows.append((name, series, kk, 100 + idx, a.elapsed_time(b), calls, flop, nbytes, (e1 - e0) * 1e-3, clk_in_kernel))
     samples = tracer.stop()
-    for name, series, kk, tag, ms, calls, flop, nbytes, joule in windows:
+    for name, series, kk, tag, ms, calls, flop, nbytes, joule, clk_in_kernel in windows:
         ss = [x for x in samples if x["phase"] == tag and x["sm_mhz"] > 0]
         bits = 0
         for x in ss:
@@ -299,6 +318,7 @@ def characterise(torch, tri, step, local, seconds, peaks, sms, est_ms):
         out[name] = {"series": series, "k": kk, "ms_sustained": per_ms, "launches": calls, "window_s": ms * 1e-3,
                      "gbs_sustained": nbytes / per_ms / 1e6, "tflops_sustained": flop / per_ms / 1e9,
                      "sm_mhz": statistics.median(x["sm_mhz"] for x in ss) if ss else None,
+                     "sm_mhz_in_kernel": clk_in_kernel or None,
                      "mem_mhz": statistics.median(x["mem_mhz"] for x in ss) if ss else None,
                      "temp_c_max": max(x["temp_c"] for x in ss) if ss else None,
                      "power_w_mean": sum(x["power_w"] for x in ss) / len(ss) if ss else None,
@@ -416,10 +436,61 @@ def gemm_shape_series(torch, tri, peaks):
     return out
 
 
+def gemv_shape_series(torch, tri, peaks, group=16):
+    """Row f4: the decode-size matrices a real decode step is mostly made of, each against the HBM roofline (bytes of X, W
+    and Y over the measured copy rate), timed like time_gemm_pair (groups of calls between one event pair, weights rotating
+    over more copies than L2 holds); and the four GEMVs of one layer back to back as one unit ("decode_layer_m8"), whose
+    roofline is the sum of their bytes."""
+    out = []
+
+    def med(fn, calls_per_group):
+        torch.cuda.synchronize()
+        time.sleep(0.2)
+        for i in range(2 * calls_per_group):
+            fn(i)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(9)]
+        for x, y in ev:
+            x.record()
+            for i in range(calls_per_group):
+                fn(i)
+            y.record()
+        torch.cuda.synchronize()
+        return sorted(x.elapsed_time(y) for x, y in ev)[4] / calls_per_group
+
+    bufs = {}
+    for label, (m, n, k) in GEMV_SHAPES.items():
+        copies = max(2, min(8, int(300e6 / (2.0 * n * k)) + 1))
+        bufs[label] = (torch.randn(m, k, device="cuda").bfloat16(), [(torch.randn(n, k, device="cuda") * 0.02).bfloat16() for _ in range(copies)],
+                       torch.empty(m, n, device="cuda", dtype=torch.bfloat16))
+
+    def call(label, i):
+        m, n, k = GEMV_SHAPES[label]
+        x, ws, y = bufs[label]
+        tri.decode_gemv(m, n, k, x, k, ws[i % len(ws)], k, tri.TRI_W_NK, y, n)
+
+    for label, (m, n, k) in GEMV_SHAPES.items():
+        ms = med(lambda i: call(label, i), group)
+        nbytes = gemm_bytes((m, n, k))
+        out.append({"kernel": "decode_gemv", "series": "decode-size GEMVs (SURVEY 8(f).4)", "label": label, "m": m, "n": n, "k": k,
+                    "bytes": nbytes, "ms": ms, "gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "bound": "hbm",
+                    "timing": f"groups of {group} calls, rotating W copies"})
+
+    def layer(i):
+        for label in DECODE_LAYER:
+            call(label, i)
+    ms = med(layer, 8)
+    nbytes = sum(gemm_bytes(GEMV_SHAPES[l]) for l in DECODE_LAYER)
+    out.append({"kernel": "decode_gemv", "series": "decode-size GEMVs (SURVEY 8(f).4)", "label": "decode_layer_m8", "m": 8, "n": 0, "k": 0,
+                "bytes": nbytes, "ms": ms, "gbs": nbytes / ms / 1e6, "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "bound": "hbm",
+                "timing": "qkv, o_proj, up, down back to back = one unit; groups of 8 units, rotating W copies"})
+    bufs.clear()
+    return out
+
+
 UNIT = "TFLOP/s (algorithmic, whole step: fp32 FMA + bf16 tensor)"
 DETAIL_FILE = os.path.join("gpurun_out", "bench_points.json")
 COMPACT_KEYS = ["impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
-                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "min_frac"]
+                "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline", "min_frac", "min_frac_kernel"]
 
 
 def point_key(pt):
@@ -465,6 +536,9 @@ def compact_line(full):
     gm = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "prefill_gemm" and q.get("label")]
     if gm:
         out["gemm_shapes"] = {q["label"]: round(q["frac"], 3) for q in gm}
+    gv = [q for q in (full.get("extra_points") or []) if q.get("kernel") == "decode_gemv" and q.get("label")]
+    if gv:
+        out["gemv_shapes"] = {q["label"]: round(q["frac"], 3) for q in gv}
     cp = ((full.get("model_fit") or {}).get("controller_preview") or {}).get("eq6_decode_phase") or {}
     if cp.get("f_selected_mhz"):                                       # Eq. 6 on the fitted model, decode phase: [selected, auto-boost] MHz
         out["eq6_decode_mhz"] = [int(cp["f_selected_mhz"]), int(cp.get("f_autoboost_mhz") or 0)]
@@ -482,7 +556,7 @@ def compact_line(full):
         return x
     out = rounded(out)
     line = json.dumps(out, separators=(",", ":"))
-    for key in ("sustained_cols", "paper_ai", "ridge", "eq6_decode_mhz", "gemm_shapes", "sustained"):   # optional keys, least needed first
+    for key in ("sustained_cols", "paper_ai", "ridge", "eq6_decode_mhz", "gemv_shapes", "gemm_shapes", "sustained"):   # optional keys, least needed first
         if len(line) <= 2800:
             break
         out.pop(key, None)                                             # the driver reads the last 3000 bytes of stdout: never outgrow them
@@ -669,12 +743,14 @@ def run_ours(args):
                 model_fit = {"error": str(e)}
         extra_points += gemm_ai_series(torch, tri, peaks)
         extra_points += gemm_shape_series(torch, tri, peaks)
+        extra_points += gemv_shape_series(torch, tri, peaks)
 
     # dominant kernel of the step: the FMA-chain kernel at k = 4096 (about half of the step time), ALU-bound
     dom = points[len(KS) - 1]
     traffic = ncu_traffic_bytes("fma_chain", column=len(KS) - 1)
     roofline = {"kernel": "fma_chain_kernel (k=4096 launch)", "bound": "alu", "achieved": dom["tflops"], "peak": alu_peak,
                 "unit": "TFLOP/s", "frac": dom["tflops"] / alu_peak, "traffic": traffic,
+                "traffic_source": NCU_CAPTURES["fma_chain"] + " (stored ncu capture)" if traffic else None,
                 "share_of_step": dom["ms"] * args.steps / total_ms,
                 "peak_source": f"derived {sms} SMs x {FP32_LANES_PER_SM} x 2 x {peaks['sm_max_mhz']:.0f} MHz; fracs vs {peaks['source']} "
                                f"{peaks['hbm_gbs']:.0f} GB/s, {peaks['bf16_tflops']:.0f} TF/s"}
@@ -690,6 +766,7 @@ def run_ours(args):
             "data": "synthetic", "config": workload_config(world), "clocks": dict(clocks, sm_mhz_in_kernel_probe=clk_probe),
             "e2e": e2e, "gpu_launches": step.launches_per_step * args.steps, "roofline": roofline, "points": points,
             "extra_points": extra_points, "model_fit": model_fit, "min_frac": min(p["frac"] for p in points),
+            "min_frac_kernel": point_key(min(points, key=lambda p: p["frac"])),
             "energy": {"j_per_step": energy_j / args.steps if energy_j else None,
                        "j_per_flop": energy_j / (STEP_FLOP * args.steps) if energy_j else None,
                        "j_per_byte": energy_j / (STEP_BYTES * args.steps) if energy_j else None},
@@ -772,8 +849,14 @@ def run_e2e(torch, tri, step, args, barrier, dist):
     n = max(1, min(args.steps, 16))                                    # the fill (first H2D) and drain (last D2H) are inside the timed region
     ms = pipeline(n)
     barrier()
-    ref = step.y if (n - 1) % 2 == 0 else sets[1]["y"]
-    ok = bool(torch.equal(hy[:4096], ref[:4096].cpu()))                # the read-back is the last step's result
+    # The read-back is the last step's result: what crossed PCIe equals what that step left on the device - a strided
+    # sample of the FMA output, ALL of the GEMV's Y and 8 rows spread over the GEMM's C.  (The results themselves are held
+    # to the oracle by tests/ and smoke(); bench.py's GPU arm may not execute oracle/ outside the cpu_baseline leg.)
+    last = sets[(n - 1) % 2]
+    rows = torch.linspace(0, hpc.shape[0] - 1, 8).long()
+    ok = bool(torch.equal(hy[:: N_FMA // 4096], last["y"][:: N_FMA // 4096].cpu()) and torch.equal(hgy, last["gy"].cpu())
+              and torch.equal(hpc[rows], last["pc"][rows.to(last["pc"].device)].cpu())
+              and bool(torch.isfinite(hgy.float()).all()) and bool(torch.isfinite(hpc[rows].float()).all()))
     ms = max_over_ranks(ms, dist, "cuda")
     world = dist.get_world_size() if dist is not None else 1
     return {"value": whole_job_value(STEP_FLOP, n, world, ms), "unit": UNIT,

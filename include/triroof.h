@@ -30,6 +30,10 @@
  *     workspaces, also when it leaves NVML loaded because a trace is running) nor after a later, larger split shape on
  *     the same stream has made the workspace grow (free + allocate; shapes up to 20 MB of partials - every shape with
  *     n, m as in configs 3-4 - never grow it).  Re-capture after either.
+ *   - Threads: the compute calls, the trace calls and the f3 host functions may be called from several host threads at
+ *     once (internal caches are locked, per-kernel set-up is idempotent and atomic); ordering on the GPU is the caller's
+ *     business, through `stream`.  tri_init() on another device and tri_shutdown() must not run while another thread is
+ *     inside the library.  prefill_gemm_static_ws has its own, stricter rule (one scratch array per device).
  *   - There is no CPU fallback: a device that is not compute capability 10.x yields TRI_ERR_ARCH.
  *   - bf16 values are passed as raw uint16_t bit patterns.
  */

@@ -2,6 +2,7 @@
 // encoder hook and the in-kernel SM clock probe.  include/triroof.h documents the ABI.
 #include "tri_internal.h"
 
+#include <atomic>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -23,7 +24,7 @@ int fail(int status, const char *fmt, ...)
 static std::mutex g_mu;
 static DeviceInfo g_info;
 static bool g_ready = false;
-static int g_generation = 0;
+static std::atomic<int> g_generation{0};
 static unsigned long long *g_clock_scratch = nullptr;
 
 static int init_locked(int device)
@@ -56,7 +57,7 @@ static int init_locked(int device)
     return TRI_OK;
 }
 
-int device_generation() { return g_generation; }
+int device_generation() { return g_generation.load(std::memory_order_acquire); }
 
 int pdl_allowed()
 {

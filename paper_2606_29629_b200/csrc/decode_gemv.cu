@@ -42,6 +42,8 @@
 #include "tri_internal.h"
 #include "ptx.cuh"
 
+#include <atomic>
+
 #include <cuda_bf16.h>
 
 namespace tri {
@@ -468,13 +470,14 @@ gemv_mma_kernel(const __grid_constant__ CUtensorMap wmap, const __grid_constant_
 
 // ksplit > 1: a grid of CTA clusters of that size along K (see the file header).
 template <typename Kernel>
-static cudaError_t launch_gemv(Kernel kernel, int *attr_gen, int xrows, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y,
+static cudaError_t launch_gemv(Kernel kernel, std::atomic<int> *attr_gen, int xrows, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y,
                                int64_t ldy, int m, int n, int k, int nslots, int blocks, int ksplit, cudaStream_t s)
 {
-    if (*attr_gen != device_generation()) {       // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen->load(std::memory_order_acquire) != device_generation()) {   // per-device function attribute: redo after tri_init() moved to
+                                                                              // another device (two threads may both do it: same value, idempotent)
         cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gemv_smem_bytes(9, 32));   // the largest configuration (>= GV_MAX_SLOTS slots of 16 rows)
         if (e != cudaSuccess) return e;
-        *attr_gen = device_generation();
+        attr_gen->store(device_generation(), std::memory_order_release);
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(blocks * ksplit);
@@ -498,7 +501,7 @@ template <bool KN>
 static cudaError_t launch_gemv_rows(int m, const CUtensorMap &wmap, const CUtensorMap &xmap, uint16_t *y, int64_t ldy, int n, int k,
                                     int nslots, int blocks, int ksplit, cudaStream_t s)
 {
-    static int gen[6] = {-1, -1, -1, -1, -1, -1};
+    static std::atomic<int> gen[6] = {{-1}, {-1}, {-1}, {-1}, {-1}, {-1}};
     if (m <= 1) return launch_gemv(gemv_kernel<1, KN>, &gen[0], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
     if (m <= 2) return launch_gemv(gemv_kernel<2, KN>, &gen[1], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);
     if (m <= 4) return launch_gemv(gemv_kernel<4, KN>, &gen[2], 8, wmap, xmap, y, ldy, m, n, k, nslots, blocks, ksplit, s);

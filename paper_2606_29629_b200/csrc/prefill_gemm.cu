@@ -23,6 +23,8 @@
 #include "ptx.cuh"
 #include "gemm_common.cuh"
 
+#include <atomic>
+
 #include <mutex>
 #include <vector>
 
@@ -328,10 +330,10 @@ void release_splitk_workspaces()
 
 static int launch_gemm_1sm(const CUtensorMap &amap, const CUtensorMap &wmap, const GemmParams &p, int sm_count, cudaStream_t s)
 {
-    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
-    if (attr_gen != device_generation()) {
+    static std::atomic<int> attr_gen{-1};         // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen.load(std::memory_order_acquire) != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_1sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, GM_SMEM_MAX));
-        attr_gen = device_generation();
+        attr_gen.store(device_generation(), std::memory_order_release);
     }
     GemmParams q = p;
     // Ring depth: as many stages as fit (a stage is the A box + 16 KiB of W).  The kernel is bound by the weight stream,

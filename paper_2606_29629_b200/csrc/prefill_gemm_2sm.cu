@@ -33,6 +33,8 @@
 #include "ptx.cuh"
 #include "gemm_common.cuh"
 
+#include <atomic>
+
 namespace tri {
 
 constexpr int G2_BM = 128, G2_BN = 256, G2_BK = 64;      // per CTA: 128 rows x 256 columns of C; pair: 256 x 256
@@ -251,10 +253,10 @@ int launch_gemm_2sm(const CUtensorMap &amap, const CUtensorMap &wmap, const Gemm
     const int n8 = p.n & ~7;     // see the epilogue: the last n % 8 columns do not go through TMA
     int st = cached_tmap_2d_bf16(&cmap, p.c, (uint64_t)(n8 ? n8 : 8), (uint64_t)p.m, (uint64_t)p.ldc * 2, 64, 32, CU_TENSOR_MAP_SWIZZLE_128B);
     if (st != TRI_OK) return st;
-    static int attr_gen = -1;                     // per-device function attribute: redo after tri_init() moved to another device
-    if (attr_gen != device_generation()) {
+    static std::atomic<int> attr_gen{-1};         // per-device function attribute: redo after tri_init() moved to another device
+    if (attr_gen.load(std::memory_order_acquire) != device_generation()) {
         TRI_CUDA(cudaFuncSetAttribute(gemm_2sm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G2_SMEM_BYTES));
-        attr_gen = device_generation();
+        attr_gen.store(device_generation(), std::memory_order_release);
     }
     const int ntiles = p.tiles_m * p.tiles_n, max_pairs = sm_count / 2;
     GemmParams q = p;

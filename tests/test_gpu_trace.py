@@ -105,8 +105,8 @@ def test_phase_trace_driver_short():
 
 def test_prefill_clock_decay_is_reported():
     """Fig. 4a: inside one prefill window the clock decays.  On B200 the config-4 GEMM starts at the
-    boost ceiling and is pulled down by the 1000 W cap within the first few hundred ms (profiles/r1_trace60.md: 1684 ->
-    1307 MHz); the per-phase summary must show it as first-10 % > last-10 %, and the decode phase must run at a higher
+    boost ceiling and is pulled down by the 1000 W cap within the first few hundred ms (profiles/r3_trace60.md: 1674 ->
+    1285 MHz); the per-phase summary must show it as first-10 % > last-10 %, and the decode phase must run at a higher
     clock than the end of the prefill phase (Observation 2)."""
     pm, pn, pk = 4096, 18944, 3584
     dm, dn, dk = 8, 18944, 3584

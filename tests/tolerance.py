@@ -8,8 +8,9 @@ SURVEY.md §8(c) S9: the stated bound is tighter than the bf16 OUTPUT rounding w
 (half an ulp of bf16 is up to 2^-9 |c| = 1.95e-3 |c|, which exceeds 1e-3 * sum|ab| once |c| > 0.51 sum|ab|);
 this happens on the tiny-K ragged-shape cases (K = 8: a single product can dominate).  No kernel that rounds
 its output to bf16 can meet it there - the oracle's own bf16 result does not.  For those cases the bound is
-widened by exactly the unavoidable part: half a bf16 ulp of the exact value plus the fp32 accumulation bound
-K * 2^-24 * sum|ab| (any summation order).  DESIGN.md lists this reading.
+widened by exactly the unavoidable part, and only on the elements where it applies (half a bf16 ulp of the exact
+value > 1e-3 * sum|ab|): half a bf16 ulp plus the fp32 accumulation bound K * 2^-24 * sum|ab| (any summation order).
+Everywhere else the stated bound holds as written, whatever K is.  DESIGN.md lists this reading.
 """
 import numpy as np
 
@@ -27,4 +28,8 @@ def stated_bound(s64: np.ndarray) -> np.ndarray:
 
 
 def widened_bound(c64: np.ndarray, s64: np.ndarray, k: int) -> np.ndarray:
-    return np.maximum(TOL * s64, half_ulp_bf16(c64) * (1.0 + 2.0 ** -6) + k * 2.0 ** -24 * s64)
+    """Reading R9 as written: the stated bound everywhere, EXCEPT on the elements where half a bf16 ulp of the exact value
+    alone exceeds it (no rounding to bf16 can meet it there); only those get half an ulp plus the fp32 accumulation term.
+    A long K (K * 2^-24 > 1e-3 from K = 16778) therefore does not loosen anything by itself."""
+    hu = half_ulp_bf16(c64)
+    return np.where(hu > TOL * s64, hu * (1.0 + 2.0 ** -6) + k * 2.0 ** -24 * s64, TOL * s64)
