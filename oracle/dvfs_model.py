@@ -9,6 +9,8 @@ clock list (the product uses the paper's binary search).  Imports nothing from p
     phase_ai(d, ai)                            Eq. 5 (line 173)
     solve_clock(...)                           Eq. 6 (line 182), exhaustive
     fit_theta(...)                             the straight-line fit stated in include/triroof.h, via numpy.polyfit
+    pace_race(sustained, f_list, prefill_s, frac)   section III-D (line 192): pace clock, pace seconds, race seconds
+    stall_clocks(entering, ...)                     section III-B (lines 130-132): what to lock on sem_wait entry / exit
 
 Pins: tests/test_oracle_dvfs.py (closed forms, limits, the paper's qualitative statements, hand-worked numbers).
 """
@@ -69,3 +71,22 @@ def fit_power(ai, f, p, eta, beta, f_sel, f_tol, p_cap):
     x = np.array([phi(a, ff, eta, beta) for a, ff in zip(ai[sel], f[sel])])
     slope, icpt = np.polyfit(x, p[sel], 1)
     return {"p_idle_w": float(icpt), "p_dyn_w": float(slope), "n_used": int(sel.sum())}
+
+
+def pace_race(sustained_mhz, f_list, prefill_s, pace_fraction=0.10):
+    """PAPER.md line 192, step by step.  "For the pace frequency, we choose the highest frequency that can run sustainably
+    across all A.I.": a clock is sustainable at an A.I. point if it does not exceed the clock that point holds in steady
+    state, so among the supported levels f_list the pace clock is the highest one that is <= EVERY entry of sustained_mhz
+    (written as that scan, not as a min).  "a pacing duration of 10% of prefill, with 90% racing": pace for
+    pace_fraction * prefill_s, then race = auto-boost for the rest.  -> (pace_mhz, pace_s, race_s); None if no level is
+    sustainable everywhere."""
+    ok = [f for f in f_list if all(f <= s for s in sustained_mhz)]
+    if not ok:
+        return None
+    return max(ok), pace_fraction * prefill_s, prefill_s - pace_fraction * prefill_s
+
+
+def stall_clocks(entering, idle_sm_mhz=210.0, idle_mem_mhz=810.0):
+    """on entering the sem_wait() of a dependency stall lock SM and memory to the clocks of the
+    lowest P8 state (210 / 810 MHz in the paper); on leaving it restore auto-boost.  -> (sm_mhz, mem_mhz, auto_boost)."""
+    return (idle_sm_mhz, idle_mem_mhz, False) if entering else (0.0, 0.0, True)

@@ -120,3 +120,39 @@ def test_fit_power_recovers_a_planted_line():
     a1, a2 = eta * 1965.0 / beta / 0.5, eta * 1965.0 / beta / 0.25          # compute-bound side: phi = eta f / (beta ai)
     g = o.fit_power([a1, a2], [1965.0, 1965.0], [865.0, 672.5], eta, beta, 1965.0, 0.0, cap)
     assert g["p_idle_w"] == pytest.approx(480.0, rel=1e-9) and g["p_dyn_w"] == pytest.approx(770.0, rel=1e-9)
+
+
+def test_pace_race_hand_worked():
+    """P:192.  Levels every 15 MHz from 1005; sustained clocks per A.I. as this repo measured them on B200 (profiles/
+    r2b_thermal240.md style): the lowest is 1657 -> the highest level not above it is 1005 + 15 * 43 = 1650.  10 % of a
+    2 s prefill = 0.2 s pacing, 1.8 s racing.  And the paper's own figure: if every A.I. sustains >= 1800 and one exactly
+    1800, the pace clock is 1800 ("we select a pace frequency of ~1800 MHz")."""
+    levels = [1005.0 + 15.0 * i for i in range(65)]                     # 1005 .. 1965
+    assert o.pace_race([1965, 1905, 1770, 1657, 1935, 1965], levels, 2.0) == (1650.0, pytest.approx(0.2), pytest.approx(1.8))
+    lv = [450.0 + 150.0 * i for i in range(18)]                         # 450 .. 3000, the paper's grid spacing
+    assert o.pace_race([2550, 1800, 2100, 1950], lv, 1.0, 0.10)[0] == 1800.0
+    assert o.pace_race([2550, 1799, 2100], lv, 1.0)[0] == 1650.0        # just below a level: the next one down
+    assert o.pace_race([400.0, 2000.0], lv, 1.0) is None                # nothing is sustainable everywhere
+    p, a, b = o.pace_race([1800.0], lv, 0.37, 0.25)
+    assert a + b == pytest.approx(0.37) and a == pytest.approx(0.0925)
+
+
+def test_pace_race_is_the_highest_common_level():
+    """Property on random inputs: the pace clock is a level, no sustained clock is below it, and the next level up (if
+    any) exceeds at least one sustained clock."""
+    rng = np.random.default_rng(7)
+    for _ in range(500):
+        lv = sorted(set(rng.integers(200, 3000, size=rng.integers(1, 40)).astype(float)))
+        sus = list(rng.uniform(150, 3100, size=rng.integers(1, 12)))
+        r = o.pace_race(sus, lv, 1.0)
+        if r is None:
+            assert min(sus) < lv[0]
+            continue
+        i = lv.index(r[0])
+        assert r[0] <= min(sus) and (i == len(lv) - 1 or lv[i + 1] > min(sus))
+
+
+def test_stall_clocks_are_the_papers():
+    assert o.stall_clocks(True) == (210.0, 810.0, False)                # P:132 "210 and 810 MHz ... lowest-level P8"
+    assert o.stall_clocks(False) == (0.0, 0.0, True)                    # "we restore auto-boost on exiting it"
+    assert o.stall_clocks(True, 345.0, 1593.0) == (345.0, 1593.0, False)
