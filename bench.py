@@ -737,6 +737,18 @@ def run_ours(args):
                     model_fit["power_at_max_clock"] = dict(pf, f_mhz=peaks["sm_max_mhz"],
                                                            source="PAPER.md Eq. 2-3 via tri_fit_power on the points at the boost ceiling, below the power cap")
                     model_fit["controller_preview"] = controller_preview(tri, fit, pf, peaks, fma_pts, points)
+                    # Row f2, second half, as a preview: the pace-and-race schedule for one config-4 prefill call from
+                    # the sustained clocks this run recorded per A.I. point and phase kernel, on the 15 MHz clock grid.  About
+                    # 1 s per point is not the paper's 240 s steady state (`characterise thermal` is), and nothing is actuated.
+                    sus = [pt["sustained"]["sm_mhz"] for pt in fma_pts + [q for q in points if q["kernel"] != "fma_chain"]
+                           if (pt.get("sustained") or {}).get("sm_mhz")]
+                    grid = [float(f) for f in range(1005, int(peaks["sm_max_mhz"]) + 1, 15)]
+                    gemm_pt = next(q for q in points if q["kernel"] == "prefill_gemm")
+                    steps = tri.tri_policy_pace_race(sus, grid, gemm_pt["ms"] * 1e-3, 0.10)
+                    model_fit["pace_race_preview"] = {"pace_mhz": steps[0]["sm_mhz"], "pace_s": steps[0]["duration_s"], "race_s": steps[1]["duration_s"],
+                                                      "sustained_mhz_min": min(sus), "points": len(sus), "actuated": False,
+                                                      "stall_idle_clocks_mhz": [tri.tri_policy_stall(True)["sm_mhz"], tri.tri_policy_stall(True)["mem_mhz"]],
+                                                      "source": "PAPER.md section III-D line 192 via tri_policy_pace_race; III-B lines 130-132 via tri_policy_stall"}
                 except tri.TriError as e:
                     model_fit["power_at_max_clock"] = {"error": str(e)}
             except tri.TriError as e:

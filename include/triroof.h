@@ -316,6 +316,33 @@ int tri_fit_theta(const double *ai, const double *f_mhz, const double *theta, si
 int tri_fit_power(const double *ai, const double *f_mhz, const double *p_w, size_t n, const tri_model *m, double f_sel_mhz,
                   double f_tol_mhz, double p_cap_w, double *p_idle_w, double *p_dyn_w, size_t *n_used);
 
+/* ------------------------------------------------------------------------------------------------
+ * f2 / f4. The two event-driven clock policies of the paper as HOST functions that only COMPUTE the schedule: nothing is
+ *     actuated here, the caller (which may hold the right to call tri_lock_clocks; tenants of a shared pool do not) applies
+ *     it.  A step with auto_boost = 1 means "release the lock" (tri_reset_clocks); otherwise lock SM (and, if mem_mhz > 0,
+ *     memory) to the given clocks.  duration_s = 0 means "until the next event".
+ */
+typedef struct {
+    double sm_mhz, mem_mhz;
+    double duration_s;
+    int32_t auto_boost;
+    int32_t reserved;
+} tri_clock_step;
+
+/* Thermal-headroom-aware pace-and-race for a high-A.I. phase (section III-D).  sustained_mhz[0..n): the
+ * SM clock each A.I. point holds in steady state (`characterise thermal` measures them).  f_mhz[0..n_f): the supported clock
+ * levels, strictly ascending.  Pace clock = "the highest frequency that can run sustainably across all A.I." = the highest
+ * level that exceeds no entry of sustained_mhz; out[0] = pace at that clock for pace_fraction * prefill_s, out[1] = race on
+ * auto-boost for the rest (the paper: pace_fraction = 0.10).  TRI_ERR_INVALID_ARG on NULL, n == 0, n_f < 1, levels not
+ * ascending, a non-positive / non-finite value, pace_fraction outside [0, 1], or when even the lowest level exceeds some
+ * sustained clock (no level is sustainable everywhere). */
+int tri_policy_pace_race(const double *sustained_mhz, size_t n, const double *f_mhz, int32_t n_f, double prefill_s,
+                         double pace_fraction, tri_clock_step out[2]);
+/* Dependency-stall-aware idle clocks (section III-B): entering != 0 is the sem_wait() entry - lock
+ * SM / memory to idle_sm_mhz / idle_mem_mhz, where a value <= 0 selects the paper's 210 / 810 MHz (the lowest P8 state);
+ * entering == 0 is the exit - restore auto-boost.  TRI_ERR_INVALID_ARG on NULL or a non-finite clock. */
+int tri_policy_stall(int entering, double idle_sm_mhz, double idle_mem_mhz, tri_clock_step *out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -40,7 +40,8 @@ EXPORTS = ["tri_status_string", "tri_last_error", "tri_init", "tri_shutdown", "t
            "roofline_run", "roofline_run_k", "decode_gemv", "prefill_gemm", "phase_trace_start", "phase_trace_mark",
            "phase_trace_stop", "phase_trace", "tri_lock_clocks", "tri_reset_clocks", "tri_nvml_sample",
            "tri_sm_clock_mhz", "tri_model_theta", "tri_model_phi", "tri_model_power", "tri_phase_ai", "tri_model_validate", "tri_solve_clock",
-           "tri_fit_theta", "tri_fit_power", "prefill_gemm_static_ws"]
+           "tri_fit_theta", "tri_fit_power", "prefill_gemm_static_ws",
+           "tri_policy_pace_race", "tri_policy_stall"]
 
 
 class TriError(RuntimeError):
@@ -53,6 +54,11 @@ class tri_model(Structure):
     """include/triroof.h tri_model (f3: PAPER.md Eq. 1-4 parameters + the P_idle / P_dyn tables on the clock list)."""
     _fields_ = [("eta", c_double), ("beta", c_double), ("omega", c_double), ("gamma", c_double), ("p_tdp", c_double),
                 ("n_f", c_int32), ("f_mhz", POINTER(c_double)), ("p_idle_w", POINTER(c_double)), ("p_dyn_w", POINTER(c_double))]
+
+
+class tri_clock_step(Structure):
+    """include/triroof.h tri_clock_step: one step of a clock schedule (auto_boost = 1: release the lock)."""
+    _fields_ = [("sm_mhz", c_double), ("mem_mhz", c_double), ("duration_s", c_double), ("auto_boost", c_int32), ("reserved", c_int32)]
 
 
 class tri_sample(Structure):
@@ -129,6 +135,8 @@ def lib():
     L.tri_solve_clock.argtypes = [POINTER(tri_model), c_double, c_double, c_double, POINTER(c_int32), POINTER(c_int32)]
     L.tri_fit_theta.argtypes = [POINTER(c_double), POINTER(c_double), POINTER(c_double), c_size_t, c_double, c_double, c_double,
                                 POINTER(tri_model)]
+    L.tri_policy_pace_race.argtypes = [POINTER(c_double), c_size_t, POINTER(c_double), c_int32, c_double, c_double, POINTER(tri_clock_step)]
+    L.tri_policy_stall.argtypes = [c_int, c_double, c_double, POINTER(tri_clock_step)]
     for name in EXPORTS:
         if getattr(L, name).restype is None and name not in ("tri_shutdown",):
             getattr(L, name).restype = c_int
@@ -357,6 +365,26 @@ def tri_fit_power(ai, f_mhz, p_w, eta, beta, f_sel_mhz, f_tol_mhz, p_cap_w):
     _check(lib().tri_fit_power((c_double * n)(*ai), (c_double * n)(*f_mhz), (c_double * n)(*p_w), n, byref(m.c), f_sel_mhz, f_tol_mhz,
                                p_cap_w, byref(pi), byref(pd), byref(used)), "tri_fit_power")
     return {"p_idle_w": pi.value, "p_dyn_w": pd.value, "n_used": used.value}
+
+
+def _step_dict(st: tri_clock_step) -> dict:
+    return {"sm_mhz": st.sm_mhz, "mem_mhz": st.mem_mhz, "duration_s": st.duration_s, "auto_boost": bool(st.auto_boost)}
+
+
+def tri_policy_pace_race(sustained_mhz, f_mhz, prefill_s: float, pace_fraction: float = 0.10) -> list:
+    """P:192 pace-and-race -> [pace step, race step] (dicts); computes the schedule only, actuates nothing."""
+    n, nf = len(sustained_mhz), len(f_mhz)
+    out = (tri_clock_step * 2)()
+    _check(lib().tri_policy_pace_race((c_double * n)(*sustained_mhz), n, (c_double * nf)(*f_mhz), nf, prefill_s, pace_fraction, out),
+           "tri_policy_pace_race")
+    return [_step_dict(out[0]), _step_dict(out[1])]
+
+
+def tri_policy_stall(entering: bool, idle_sm_mhz: float = 0.0, idle_mem_mhz: float = 0.0) -> dict:
+    """P:130-132 stall-aware idle clocks -> one step (dict); computes only."""
+    out = tri_clock_step()
+    _check(lib().tri_policy_stall(int(bool(entering)), idle_sm_mhz, idle_mem_mhz, byref(out)), "tri_policy_stall")
+    return _step_dict(out)
 
 
 # the C names of the row-f3 entry points, on a Model

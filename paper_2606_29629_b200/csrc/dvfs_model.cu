@@ -186,4 +186,43 @@ int tri_fit_power(const double *ai, const double *f_mhz, const double *p_w, size
     return TRI_OK;
 }
 
+int tri_policy_pace_race(const double *sustained_mhz, size_t n, const double *f_mhz, int32_t n_f, double prefill_s,
+                         double pace_fraction, tri_clock_step out[2])
+{
+    if (!sustained_mhz || !f_mhz || !out || n == 0 || n_f < 1) return tri::fail(TRI_ERR_INVALID_ARG, "NULL argument, n == 0 or n_f < 1");
+    if (!(prefill_s >= 0.0) || !std::isfinite(prefill_s) || !(pace_fraction >= 0.0 && pace_fraction <= 1.0))
+        return tri::fail(TRI_ERR_INVALID_ARG, "prefill_s must be >= 0 and pace_fraction in [0, 1]");
+    // the clock every A.I. point can hold: the lowest of the sustained clocks
+    double floor_mhz = INFINITY;
+    for (size_t i = 0; i < n; ++i) {
+        if (!tri::pos(sustained_mhz[i])) return tri::fail(TRI_ERR_INVALID_ARG, "sustained_mhz[%zu] is not positive and finite", i);
+        if (sustained_mhz[i] < floor_mhz) floor_mhz = sustained_mhz[i];
+    }
+    for (int32_t i = 0; i < n_f; ++i)
+        if (!tri::pos(f_mhz[i]) || (i > 0 && !(f_mhz[i] > f_mhz[i - 1])))
+            return tri::fail(TRI_ERR_INVALID_ARG, "f_mhz must be positive and strictly ascending (index %d)", (int)i);
+    if (f_mhz[0] > floor_mhz)
+        return tri::fail(TRI_ERR_INVALID_ARG, "no supported clock is sustainable at every A.I. (lowest level %g MHz > %g MHz)", f_mhz[0], floor_mhz);
+    // highest level <= floor_mhz: bisection over the ascending table (f_mhz[lo] <= floor_mhz < f_mhz[hi])
+    int32_t lo = 0, hi = n_f;
+    while (hi - lo > 1) {
+        const int32_t mid = lo + (hi - lo) / 2;
+        if (f_mhz[mid] <= floor_mhz) lo = mid;
+        else hi = mid;
+    }
+    const double pace_s = pace_fraction * prefill_s;
+    out[0] = tri_clock_step{f_mhz[lo], 0.0, pace_s, 0, 0};
+    out[1] = tri_clock_step{0.0, 0.0, prefill_s - pace_s, 1, 0};
+    return TRI_OK;
+}
+
+int tri_policy_stall(int entering, double idle_sm_mhz, double idle_mem_mhz, tri_clock_step *out)
+{
+    if (!out) return tri::fail(TRI_ERR_INVALID_ARG, "out is NULL");
+    if (!std::isfinite(idle_sm_mhz) || !std::isfinite(idle_mem_mhz)) return tri::fail(TRI_ERR_INVALID_ARG, "idle clocks must be finite");
+    if (entering) *out = tri_clock_step{idle_sm_mhz > 0.0 ? idle_sm_mhz : 210.0, idle_mem_mhz > 0.0 ? idle_mem_mhz : 810.0, 0.0, 0, 0};
+    else *out = tri_clock_step{0.0, 0.0, 0.0, 1, 0};
+    return TRI_OK;
+}
+
 }  // extern "C"

@@ -143,3 +143,42 @@ def test_power_fit_matches_oracle_and_recovers_planted_line():
         assert got[key] == pytest.approx(want[key], rel=1e-8), key
     with pytest.raises(tri.TriError):
         tri.tri_fit_power(list(ai), list(f), list(noisy), eta, beta, 1000.0, 1.0, 990.0)      # no point at that clock
+
+
+def test_pace_race_equals_the_oracle():
+    """P:192 through the C ABI against oracle.pace_race (a scan over the levels; the library bisects) on random level tables and
+    sustained clocks, the refusal included; plus the hand-worked B200 case (1657 MHz floor -> 1650 MHz, 0.2 s + 1.8 s)."""
+    rng = np.random.default_rng(21)
+    refused = 0
+    for _ in range(2000):
+        lv = sorted(set(rng.integers(200, 3000, size=rng.integers(1, 60)).astype(float)))
+        sus = [float(x) for x in rng.uniform(150, 3100, size=rng.integers(1, 12))]
+        if rng.random() < 0.3:
+            sus[0] = float(rng.choice(lv))                          # a sustained clock exactly on a level
+        prefill, frac = float(rng.uniform(0.0, 5.0)), float(rng.choice([0.0, 0.1, 0.25, 1.0]))
+        want = o.pace_race(sus, lv, prefill, frac)
+        if want is None:
+            with pytest.raises(tri.TriError):
+                tri.tri_policy_pace_race(sus, lv, prefill, frac)
+            refused += 1
+            continue
+        pace, race = tri.tri_policy_pace_race(sus, lv, prefill, frac)
+        assert pace["sm_mhz"] == want[0] and not pace["auto_boost"] and race["auto_boost"] and race["sm_mhz"] == 0.0
+        assert pace["duration_s"] == pytest.approx(want[1], abs=1e-12) and race["duration_s"] == pytest.approx(want[2], abs=1e-12)
+    assert 20 < refused < 1500
+    levels = [1005.0 + 15.0 * i for i in range(65)]
+    pace, race = tri.tri_policy_pace_race([1965, 1905, 1770, 1657, 1935, 1965], levels, 2.0)
+    assert (pace["sm_mhz"], round(pace["duration_s"], 9), round(race["duration_s"], 9)) == (1650.0, 0.2, 1.8)
+    for bad in [([], levels, 1.0, 0.1), ([1800.0], [], 1.0, 0.1), ([1800.0], [900.0, 900.0], 1.0, 0.1), ([1800.0], levels, -1.0, 0.1),
+                ([1800.0], levels, 1.0, 1.5), ([float("nan")], levels, 1.0, 0.1)]:
+        with pytest.raises(tri.TriError):
+            tri.tri_policy_pace_race(*bad)
+
+
+def test_stall_policy_equals_the_oracle():
+    for args in [(True,), (False,), (True, 345.0, 1593.0), (True, 345.0, 0.0)]:
+        got = tri.tri_policy_stall(*args)
+        sm, mem, boost = o.stall_clocks(args[0], *[a if a > 0 else d for a, d in zip(args[1:], (210.0, 810.0))]) if len(args) > 1 else o.stall_clocks(args[0])
+        assert (got["sm_mhz"], got["mem_mhz"], got["auto_boost"], got["duration_s"]) == (sm, mem, boost, 0.0)
+    with pytest.raises(tri.TriError):
+        tri.tri_policy_stall(True, float("inf"), 0.0)
